@@ -1,0 +1,350 @@
+"""Physics pins for the CPU oracle: closed forms and exact invariants of whole steps (P4, P6-P9, P11-P14).
+
+Each test states the mathematical fact it leans on; tolerances are the ones DESIGN.md section 4 derives.  CPU only.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2505_01126_b200 import workloads as wl
+
+import naive_numpy as nv
+
+CS2 = 1.0 / 3.0
+
+
+def run(cfg, steps, shape=None):
+    n = cfg["n"]
+    nx, ny, nz = shape or (n, n, n)
+    o = oracle.Oracle(nx, ny, nz, **cfg["params"])
+    o.init(cfg["rho"], cfg["u"], cfg["phi"])
+    o.step(steps)
+    return o
+
+
+# ------------------------------------------------------------------ P7: special cases of one step
+def test_p7_uniform_state_is_fixed_point():
+    n = 6
+    o = oracle.Oracle(n, n, n, tau=0.7)
+    rho = np.full((n, n, n), 1.3)
+    u = np.zeros((3, n, n, n))
+    u[0], u[1], u[2] = 0.03, -0.02, 0.05
+    o.init(rho, u)
+    f0 = o.populations()
+    o.step(5)
+    assert np.abs(o.populations() - f0).max() < 1e-15
+    r, uu, _ = o.moments()
+    assert np.abs(r - 1.3).max() < 1e-15 and np.abs(uu - u).max() < 1e-15
+
+
+def test_p7_tau_one_gives_equilibrium_plus_half_force():
+    """omega = 1: Eq. 6 reduces to f_i(x + c_i, t+1) = f_i^eq + S_i/2, whatever the incoming non-equilibrium."""
+    rng = np.random.default_rng(7)
+    nx, ny, nz = 5, 6, 7
+    p = dict(tau=1.0, force_type=1, force_amp=1e-3, force_k=1)
+    o = oracle.Oracle(nx, ny, nz, **p)
+    _, w = oracle.lattice()
+    f = w[:, None, None, None] * (1 + 0.05 * rng.standard_normal((27, nz, ny, nx)))
+    o.set_populations(f)
+    pst, u, _ = o.moments()
+    A = o.accel()
+    o.step(1)
+    f1 = o.populations()
+    c, _ = oracle.lattice()
+    for i in (0, 5, 13, 14, 22, 26):
+        for (x, y, z) in [(0, 0, 0), (4, 5, 6), (2, 3, 1)]:
+            xs, ys, zs = (x - c[i][0]) % nx, (y - c[i][1]) % ny, (z - c[i][2]) % nz
+            ref = oracle.feq(pst[zs, ys, xs], u[:, zs, ys, xs])[i] + 0.5 * oracle.guo(u[:, zs, ys, xs], A[:, zs, ys, xs])[i]
+            assert abs(f1[i, z, y, x] - ref) < 1e-16
+
+
+# ------------------------------------------------------------------ P13: brute-force second evaluation
+@pytest.mark.parametrize("two_phase,ratio", [(0, 1.0), (1, 1.0), (1, 10.0)])
+def test_p13_oracle_equals_naive_collide_push(two_phase, ratio):
+    """Pull/two-pass oracle (Eq. 6) == collide-at-node BGK on Hermite-projected populations + push (Eq. 4),
+    on an anisotropic box (8 x 10 x 12) so that any axis or sign mix-up shows."""
+    rng = np.random.default_rng(13)
+    nx, ny, nz = 8, 10, 12
+    p = dict(tau=0.6, two_phase=two_phase, rho_l=ratio, rho_g=1.0, sigma=0.01, mobility=0.05, width=4.0,
+             force_type=1, force_amp=1e-4, force_k=1)
+    Z, Y, X = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    rho = 1.0 + 0.01 * rng.standard_normal((nz, ny, nx))
+    u = 0.02 * rng.standard_normal((3, nz, ny, nx))
+    r = np.sqrt((X - 3.3) ** 2 + (Y - 4.1) ** 2 + (Z - 5.7) ** 2)
+    phi = 0.5 * (1 + np.tanh(2 * (3.0 - r) / 4.0)) if two_phase else None
+    o = oracle.Oracle(nx, ny, nz, **p)
+    o.init(rho, u, phi)
+    f = nv.init(rho, u, phi, p)
+    assert np.abs(o.populations() - f).max() < 1e-15
+    ph = phi
+    for _ in range(3):
+        f, ph = nv.step(f, ph, p)
+    o.step(3)
+    assert np.abs(o.populations() - f).max() < 1e-14
+    r_o, u_o, phi_o = o.moments()
+    r_n, u_n, *_ = nv.moments(f, ph, p)
+    assert np.abs(r_o - r_n).max() < 1e-14 and np.abs(u_o - u_n).max() < 1e-14
+    if two_phase:
+        assert np.abs(phi_o - ph).max() < 1e-14
+
+
+# ------------------------------------------------------------------ forcing closed forms (Eq. 5, R3, R4)
+def test_uniform_acceleration_is_exact():
+    """ABC forcing with k_f = 0 is the uniform force A(1,1,1): a uniform fluid accelerates as u(t) = u0 + A t with
+    no error term (pins sum_i S_i c_i = A and the half-force in u, R4)."""
+    n = 4
+    o = oracle.Oracle(n, n, n, tau=0.9, force_type=1, force_amp=1e-4, force_k=0)
+    u0 = np.zeros((3, n, n, n))
+    u0[0] = 0.01
+    o.init(np.ones((n, n, n)), u0)
+    for t in (0, 1, 7):
+        _, u, _ = o.moments()
+        assert np.abs(u[0] - (0.01 + 1e-4 * t)).max() < 1e-15
+        assert np.abs(u[1] - 1e-4 * t).max() < 1e-15
+        o.step(1 if t == 0 else 6)
+
+
+def test_kolmogorov_flow_steady_state():
+    """F_x = F0 sin(k y): steady Stokes solution u_x = F0 sin(k y) / (nu k^2), nu = cs2 (tau - 1/2).
+    Sine forcing (type 2) drives three such decoupled shear flows; amplitude is kept tiny so u.grad u ~ 1e-14."""
+    n, tau, F0 = 16, 1.0, 1e-9
+    nu = CS2 * (tau - 0.5)
+    k = 2 * np.pi / n
+    o = oracle.Oracle(n, n, n, tau=tau, force_type=2, force_amp=F0, force_k=1)
+    o.init(np.ones((n, n, n)), np.zeros((3, n, n, n)))
+    o.step(int(12 / (nu * k * k)))          # e^-12 of the transient left
+    _, u, _ = o.moments()
+    y = np.arange(n)
+    expect = F0 * np.sin(k * y) / (nu * k * k)
+    got = u[0][0, :, 0]
+    assert np.abs(got - expect).max() / np.abs(expect).max() < 0.015   # O(k^2) lattice correction, k^2/12 = 1.3 %
+    assert np.abs(u[0] - got[None, :, None]).max() < 1e-5 * np.abs(expect).max()   # u_x depends on y only (u.grad u ~ 1e-14)
+
+
+# ------------------------------------------------------------------ P6 / P14: Taylor-Green vortex (config 1)
+@pytest.fixture(scope="module")
+def tgv_history():
+    cfg = wl.make_config("tgv")
+    o = oracle.Oracle(32, 32, 32, **cfg["params"])
+    o.init(cfg["rho"], cfg["u"])
+    hist = [o.diagnostics()]
+    for _ in range(10):
+        o.step(10)
+        hist.append(o.diagnostics())
+    return o, hist
+
+
+def test_p6_tgv_energy_decay_rate(tgv_history):
+    """E(t) = E(0) exp(-2 nu k^2 t), k^2 = 3 (2 pi / 32)^2, nu = (0.8 - 0.5)/3 = 0.1 (Stokes limit, Re ~ 1)."""
+    _, hist = tgv_history
+    nu, k2 = 0.1, 3 * (2 * np.pi / 32) ** 2
+    t = np.array([h["step"] for h in hist])
+    E = np.array([h["ke"] for h in hist])
+    assert abs(E[0] - 0.02 ** 2 / 8) < 1e-18          # <|u|^2>/2 of the TGV field = U0^2 / 8
+    sel = t >= 20                                      # skip the equilibrium-initialisation transient (R15)
+    rate = -np.polyfit(t[sel], np.log(E[sel]), 1)[0]
+    assert abs(rate / (2 * nu * k2) - 1) < 0.01
+    assert abs(E[-1] / E[0] / np.exp(-2 * nu * k2 * 100) - 1) < 0.03
+
+
+def test_p6_dissipation_diagnostic_is_minus_dEdt(tgv_history):
+    """R21: eps = nu a:a / (2 cs4 tau^2) equals 2 nu k^2 E on the decaying vortex (uses a = -cs2 tau (du+du^T), L94)."""
+    _, hist = tgv_history
+    nu, k2 = 0.1, 3 * (2 * np.pi / 32) ** 2
+    for h in hist[3:]:
+        assert abs(h["dissipation"] / (2 * nu * k2 * h["ke"]) - 1) < 0.02
+
+
+def test_p14_hermite_coefficient_is_strain(tgv_history):
+    """a_ab = -cs2 tau (d_a u_b + d_b u_a) + O(Ma^3), gradient by the lattice stencil."""
+    o, _ = tgv_history
+    _, u, _ = o.moments()
+    a = o.hermite()
+    du = np.stack([oracle.gradient(u[b]) for b in range(3)], axis=1)   # du[a, b] = d_a u_b
+    idx = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+    scale = CS2 * 0.8 * np.abs(du).max()
+    for j, (al, be) in enumerate(idx):
+        expect = -CS2 * 0.8 * (du[al, be] + du[be, al])
+        assert np.abs(a[j] - expect).max() < 0.05 * scale
+
+
+def test_p4_tgv_mass_and_momentum(tgv_history):
+    _, hist = tgv_history
+    assert abs(hist[-1]["sum_pstar"] / hist[0]["sum_pstar"] - 1) < 1e-12
+    for k in ("sum_mx", "sum_my", "sum_mz"):
+        assert abs(hist[-1][k] - hist[0][k]) < 1e-12
+
+
+# ------------------------------------------------------------------ P4: conservation under forcing, turbulent-like field
+def test_p4_forced_hit_conserves_mass_and_momentum():
+    cfg = wl.make_config("hit", n=16)
+    o = run(cfg, 0)
+    d0 = o.diagnostics()
+    o.step(60)
+    d1 = o.diagnostics()
+    assert abs(d1["sum_pstar"] / d0["sum_pstar"] - 1) < 1e-12
+    for k in ("sum_mx", "sum_my", "sum_mz"):          # sum_x F^b = 0 (R20) -> total momentum unchanged
+        assert abs(d1[k] - d0[k]) < 1e-12
+    assert np.isfinite(d1["ke"]) and d1["ke"] > 0
+
+
+def test_p4_momentum_balance_two_phase():
+    """sum_x m(t+1) - sum_x m(t) = sum_x F/rho(t): Guo forcing injects exactly A per node per step."""
+    cfg = wl.make_config("droplet", n=16, density_ratio=10.0)
+    cfg["params"].update(force_type=1, force_amp=1e-5)
+    o = run(cfg, 3)
+    d0 = o.diagnostics()
+    A = o.accel()
+    o.step(1)
+    d1 = o.diagnostics()
+    for al, k in enumerate(("sum_mx", "sum_my", "sum_mz")):
+        assert abs((d1[k] - d0[k]) - A[al].sum()) < 1e-13
+    assert abs(d1["sum_pstar"] - d0["sum_pstar"]) < 1e-12 * 16 ** 3   # zero-gauge run: absolute (R26)
+
+
+# ------------------------------------------------------------------ P8 / P9: Allen-Cahn
+def test_p8_total_phi_conserved_under_advection():
+    cfg = wl.make_config("bubbly", n=24)
+    cfg["phi"] = wl.droplet_phi(24, 6.0)
+    o = run(cfg, 0)
+    s0 = o.diagnostics()["sum_phi"]
+    o.step(40)
+    d = o.diagnostics()
+    assert abs(d["sum_phi"] / s0 - 1) < 1e-12
+    _, _, phi = o.moments()
+    assert phi.min() > -0.02 and phi.max() < 1.05            # boundedness sanity (R = 6 is barely resolved)
+
+
+def test_p9_flat_interface_relaxes_to_tanh_profile():
+    """Steady 1-D solution of Eq. 3 with kappa = 4D/delta: D phi' = kappa phi (1 - phi)  ->
+    phi = (1 + tanh(2 xi / delta)) / 2 (R10).  Start from a too-sharp slab and let it relax."""
+    nx, ny, nz, W = 64, 4, 4, 4.0
+    x = np.arange(nx) - (nx - 1) / 2
+    prof = lambda w: 0.5 * (np.tanh(2 * (x + 16) / w) - np.tanh(2 * (x - 16) / w))
+    phi = np.broadcast_to(prof(2.0), (nz, ny, nx)).copy()
+    p = dict(tau=0.8, two_phase=1, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.05, width=W)
+    o = oracle.Oracle(nx, ny, nz, **p)
+    o.init(np.ones((nz, ny, nx)), np.zeros((3, nz, ny, nx)), phi)
+    s0 = o.diagnostics()["sum_phi"]
+    o.step(4000)
+    _, u, ph = o.moments()
+    assert abs(o.diagnostics()["sum_phi"] / s0 - 1) < 1e-12
+    # conserved sum fixes the slab half-width; compare against the closed form with that half-width
+    half = ph[0, 0].sum() / 2
+    expect = 0.5 * (np.tanh(2 * (x + half) / W) - np.tanh(2 * (x - half) / W))
+    assert np.abs(ph[0, 0] - expect).max() < 1e-2
+    assert np.abs(ph - ph[0:1, 0:1]).max() < 1e-14      # stays one-dimensional
+    assert np.abs(u).max() < 1e-12                        # sigma = 0, equal densities: no flow
+
+
+# ------------------------------------------------------------------ P11: Laplace law
+def laplace_ratio(o, n2d_or_3d, R_eff, sigma, rho_l, rho_g, centre, far):
+    r, _, phi = o.moments()
+    rho = rho_g + (rho_l - rho_g) * phi
+    p = CS2 * rho * r                                   # p = p* rho cs2
+    dp = p[centre] - p[far]
+    return dp / (n2d_or_3d * sigma / R_eff)
+
+
+def test_p11_laplace_cylinder():
+    """z-invariant droplet (nz = 1): Delta p = sigma / R.  Pins the 3 delta / 2 normalisation and the sign of F^s (R8)."""
+    n, R, sigma = 64, 16.0, 0.01
+    ax = np.arange(n) - (n - 1) / 2
+    Y, X = np.meshgrid(ax, ax, indexing="ij")
+    phi = (0.5 * (1 + np.tanh(2 * (R - np.sqrt(X * X + Y * Y)) / 4.0)))[None]
+    p = dict(tau=0.8, two_phase=1, rho_l=1.0, rho_g=1.0, sigma=sigma, mobility=0.05, width=4.0)
+    o = oracle.Oracle(n, n, 1, **p)
+    o.init(np.ones((1, n, n)), np.zeros((3, 1, n, n)), phi)
+    ratios = []
+    for _ in range(10):
+        o.step(300)
+        R_eff = np.sqrt(o.diagnostics()["sum_phi"] / np.pi)
+        ratios.append(laplace_ratio(o, 1.0, R_eff, sigma, 1.0, 1.0, (0, n // 2, n // 2), (0, 0, 0)))
+    assert abs(np.mean(ratios[4:]) - 1) < 0.05, ratios
+    assert o.diagnostics()["umax"] < 1e-4               # spurious currents
+
+
+@pytest.mark.parametrize("ratio,gauge", [(1.0, 1.0), (10.0, 0.0)])
+def test_p11_laplace_sphere(ratio, gauge):
+    """3-D droplet: Delta p = 2 sigma / R_eff, R_eff = (3 sum phi / 4 pi)^(1/3); density ratio 10 uses zero gauge
+    pressure (R26) and exercises A = F/rho (R3), F^p and F^nu (R9)."""
+    n, R, sigma = 32, 9.0, 0.01
+    cfg = wl.make_config("droplet", n=n, density_ratio=ratio)
+    cfg["phi"] = wl.droplet_phi(n, R)
+    o = run(cfg, 0)
+    ratios = []
+    for _ in range(8):
+        o.step(100)
+        R_eff = (3 * o.diagnostics()["sum_phi"] / (4 * np.pi)) ** (1 / 3)
+        ratios.append(laplace_ratio(o, 2.0, R_eff, sigma, ratio, 1.0, (n // 2,) * 3, (0, 0, 0)))
+    assert abs(np.mean(ratios[3:]) - 1) < 0.10, ratios
+    assert o.diagnostics()["umax"] < 2e-4
+
+
+# ------------------------------------------------------------------ P12: lattice symmetries
+def _two_phase_case(n=12, seed=12):
+    rng = np.random.default_rng(seed)
+    ax = np.arange(n)
+    Z, Y, X = np.meshgrid(ax, ax, ax, indexing="ij")
+    r = np.sqrt((X - 4.0) ** 2 + (Y - 6.5) ** 2 + (Z - 5.0) ** 2)
+    phi = 0.5 * (1 + np.tanh(2 * (3.5 - r) / 4.0))
+    u = 0.02 * rng.standard_normal((3, n, n, n))
+    rho = 1 + 0.01 * rng.standard_normal((n, n, n))
+    p = dict(tau=0.55, two_phase=1, rho_l=3.0, rho_g=1.0, sigma=0.01, mobility=0.05, width=4.0)
+    return p, rho, u, phi
+
+
+def _advance(p, rho, u, phi, steps=4):
+    n = rho.shape[0]
+    o = oracle.Oracle(n, n, n, **p)
+    o.init(rho, u, phi)
+    o.step(steps)
+    return o.moments()
+
+
+def test_p12_periodic_shift_is_bitwise():
+    p, rho, u, phi = _two_phase_case()
+    base = _advance(p, rho, u, phi)
+    sh = dict(shift=(5, -3, 7), axis=(-3, -2, -1))
+    moved = _advance(p, np.roll(rho, **sh), np.roll(u, **sh), np.roll(phi, **sh))
+    for b, m in zip(base, moved):
+        assert np.array_equal(np.roll(b, **sh), m)
+
+
+def test_p12_axis_permutation_and_reflection():
+    """x->y->z->x relabelling and the mirror x -> -x map solutions to solutions (no body force)."""
+    p, rho, u, phi = _two_phase_case()
+    r0, u0, f0 = _advance(p, rho, u, phi)
+    # cyclic permutation: new field g(z,y,x) = old(y,x,z)  <=> transpose axes; vector components permute alike
+    perm = (1, 2, 0)                                  # new axes (z',y',x') take old axes (y,x,z)
+    tp = lambda s: np.transpose(s, perm)
+    # old comps (ux,uy,uz) live on axes (2,1,0); after the transpose old axis y -> z', x -> y', z -> x'
+    u_new = np.stack([tp(u[2]), tp(u[0]), tp(u[1])])  # (ux', uy', uz') = (uz, ux, uy)
+    r1, u1, f1 = _advance(p, tp(rho), u_new, tp(phi))
+    assert np.abs(tp(r0) - r1).max() < 1e-13 and np.abs(tp(f0) - f1).max() < 1e-13
+    assert np.abs(np.stack([tp(u0[2]), tp(u0[0]), tp(u0[1])]) - u1).max() < 1e-13
+    # reflection in x
+    fl = lambda s: s[..., ::-1]
+    u_ref = np.stack([-fl(u[0]), fl(u[1]), fl(u[2])])
+    r2, u2, f2 = _advance(p, fl(rho), u_ref, fl(phi))
+    assert np.abs(fl(r0) - r2).max() < 1e-13 and np.abs(fl(f0) - f2).max() < 1e-13
+    assert np.abs(np.stack([-fl(u0[0]), fl(u0[1]), fl(u0[2])]) - u2).max() < 1e-13
+
+
+# ------------------------------------------------------------------ sub-box evaluation used by the full-size GPU parity test
+def test_subbox_evaluation_matches_full_box_interior():
+    """k steps only depend on inputs within radius 3k (two-phase) of a node: running the oracle on a periodic
+    sub-box reproduces the full-box values away from the sub-box rim."""
+    n, s, k = 24, 18, 2
+    cfg = wl.make_config("bubbly", n=n)
+    cfg["phi"] = wl.bubbles_phi(n, np.array([[9.0, 10.0, 11.0]]), radius=5.0)
+    full = run(cfg, k).moments()
+    org = (20, 3, 15)                                   # wraps across the periodic boundary in x
+    sub = oracle.Oracle(s, s, s, **cfg["params"], force_period=(n, n, n), force_origin=org)
+    sub.init(wl.subbox(cfg["rho"], org, s), wl.subbox(cfg["u"], org, s), wl.subbox(cfg["phi"], org, s))
+    sub.step(k)
+    got = sub.moments()
+    rim = 3 * k + 2
+    inner = (slice(rim, s - rim),) * 3
+    for a, b in zip(full, got):
+        assert np.abs(wl.subbox(a, org, s)[..., inner[0], inner[1], inner[2]] - b[..., inner[0], inner[1], inner[2]]).max() < 1e-15
