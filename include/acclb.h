@@ -1,0 +1,126 @@
+/*
+ * acclb.h -- C ABI of libacclb.so: the per-time-step lattice update of accLB (arXiv 2505.01126) on one
+ * NVIDIA B200 (sm_100a).  Citations are PAPER.md:Lnn (+ equation) of /root/reference/PAPER.md; "Rnn" are the
+ * readings of the paper listed in DESIGN.md section 2.
+ *
+ * What the library computes (one step t -> t+1, fully periodic box, lattice units dx = dt = 1, fp64):
+ *   thread-safe regularized D3Q27 lattice-Boltzmann collide+stream of the hydrodynamic populations
+ *     f_i(x + c_i, t+1) = f_i^eq + (1 - omega) f_i^neq + S_i / 2                 PAPER.md:L85  (Eq. 6)
+ *   with the pressure-based equilibrium and second-order Hermite reconstruction  PAPER.md:L88-92 (Eq. 7)
+ *   and Guo forcing S_i                                                          PAPER.md:L79  (Eq. 5),
+ *   coupled (two_phase = 1) to the conservative Allen-Cahn equation              PAPER.md:L61  (Eq. 3)
+ *   discretised with WENO5 advection and lattice stencils
+ *   and to the interface force F = F^s + F^p + F^nu                              PAPER.md:L100 (Eq. 8).
+ *
+ * Conventions
+ *   - Plain pointers and sizes only.  Every pointer argument says HOST or DEVICE.
+ *   - Field layout: scalars [nz][ny][nx] with x fastest; vectors [3][nz][ny][nx], component 0 = x.
+ *   - "rho" in this API is the zeroth moment p* = sum_i f_i (the conserved "mass", R19); the mixture density
+ *     is rho(phi) = rho_g + (rho_l - rho_g) phi.
+ *   - The library never allocates or frees device memory: the caller (PyTorch) passes ONE workspace block of
+ *     accLB_workspace_bytes() bytes, 256-byte aligned, that must outlive the context.  It never frees caller
+ *     memory.  All work is enqueued on params.stream of device params.device.
+ *   - Return value 0 = ACCLB_OK, negative = error; accLB_last_error() gives the text (thread-local).
+ *   - A context is not thread-safe; distinct contexts are independent ("replicas only" across GPUs).
+ *   - There is no CPU fallback: every entry point needs a CUDA device.
+ */
+#ifndef ACCLB_H
+#define ACCLB_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ACCLB_OK 0
+#define ACCLB_EINVAL (-1)     /* bad size / parameter / NULL pointer                      */
+#define ACCLB_EWORKSPACE (-2) /* workspace too small or not 256-byte aligned              */
+#define ACCLB_ECUDA (-3)      /* CUDA runtime / launch error, text in accLB_last_error()  */
+#define ACCLB_ENUMERIC (-4)   /* a diagnostic is not finite                               */
+
+#define ACCLB_NDIAG 9 /* length of the accLB_diagnostics vector */
+
+typedef struct accLB_ctx accLB_ctx; /* opaque; owned by the library; freed by accLB_destroy */
+
+/* POD, copied at create; no pointer is kept except `stream`. */
+typedef struct {
+  double tau;       /* relaxation time > 0.5; nu = (tau - 1/2)/3, omega = 1/tau      */
+  int two_phase;    /* 0: single component (rho == 1, phi ignored); 1: LB + Allen-Cahn   */
+  double rho_l;     /* density where phi = 1 (R16)     */
+  double rho_g;     /* density where phi = 0                                                               */
+  double sigma;     /* surface tension gamma */
+  double mobility;  /* D of Eq. 3 (BASELINE "M")      */
+  double width;     /* interface width delta (BASELINE "W"); kappa = 4 D / delta      */
+  int force_type;   /* 0 none | 1 ABC: A(sin kz + cos ky, sin kx + cos kz, sin ky + cos kx) PAPER.md:L167
+                       | 2 sine: F0 (sin ky, sin kz, sin kx) (BASELINE config 2); R20                      */
+  double force_amp; /* A or F0 (a force density: divided by rho(phi) like the other forces, R3)            */
+  int force_k;      /* forcing wavenumber in units of 2 pi / L per axis                                    */
+  int store_fp32;   /* 0: populations stored fp64; 1: stored as float(f_i - w_i), arithmetic fp64 (R22)    */
+  int host_staging; /* 1: workspace also holds 5 n doubles of staging so accLB_run_host can be used        */
+  int device;       /* CUDA device ordinal                                                                 */
+  void* stream;     /* cudaStream_t of the caller (NULL = legacy default stream)                           */
+} accLB_params;
+
+/* Bytes of device workspace accLB_create needs for this grid and these parameters; 0 on invalid arguments
+ * (nx, ny, nz >= 4, nx even, nx*ny*nz < 2^31, tau > 0.5, two_phase: rho_l, rho_g > 0, width > 0). */
+size_t accLB_workspace_bytes(int nx, int ny, int nz, const accLB_params* params);
+
+/* Create a context on `workspace` (DEVICE pointer, caller-owned, 256-byte aligned, >= workspace_bytes).
+ * Builds the body-force tables (R20) on the host with libm and uploads them.  *out is set on success. */
+int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* params, void* workspace,
+                 size_t workspace_bytes);
+
+/* Initial state (R15): f_i = f_i^eq(p*, u0) - S_i(u0, A)/2 with A from F^s + F^p + F^b, step counter := 0.
+ * rho, u, phi: DEVICE pointers, caller-owned, read-only, fp64; phi may be NULL when two_phase = 0.
+ * Enqueues on the stream; the inputs must stay valid until the stream reaches that point. */
+int accLB_init(accLB_ctx* ctx, const double* rho, const double* u, const double* phi);
+
+/* Advance nsteps >= 0 time steps (rows a1-a8 of DESIGN.md section 1).  Enqueues only; does not synchronise. */
+int accLB_step(accLB_ctx* ctx, int nsteps);
+
+/* Macroscopic fields of the current state: rho := p* = sum f_i, u = sum f_i c_i + A/2 (R4),
+ * phi.  DEVICE pointers, caller-owned, written; any may be NULL (phi is ignored when two_phase = 0).
+ * The state is unchanged.  Enqueues only. */
+int accLB_moments(accLB_ctx* ctx, double* rho, double* u, double* phi);
+
+/* Diagnostics of the current state (R21) into out[0..ACCLB_NDIAG-1] (HOST pointer, n_out >= ACCLB_NDIAG):
+ *   0 KE = <rho(phi) |u|^2 / 2>      1 dissipation = <nu a:a / (2 cs^4 tau^2)>
+ *   2 sum phi   3 sum p*   4..6 sum_x sum_i f_i c_i   7 max |u|   8 step count.
+ * Warp-shuffle + one atomic per block and quantity.  Synchronises the stream.  ACCLB_ENUMERIC if non-finite. */
+int accLB_diagnostics(accLB_ctx* ctx, double* out, int n_out);
+
+/* The same path fed from HOST buffers (what an application without device arrays calls; bench.py's e2e leg):
+ * copy rho,u,phi host->device (staging), accLB_init, accLB_step(nsteps), accLB_moments, copy the three fields
+ * device->host, optionally diagnostics.  Needs params.host_staging = 1.  h_* are HOST pointers (pinned memory
+ * makes the copies asynchronous); outputs and h_diag (ACCLB_NDIAG doubles) may be NULL.  Synchronises. */
+int accLB_run_host(accLB_ctx* ctx, const double* h_rho, const double* h_u, const double* h_phi, int nsteps,
+                   double* h_rho_out, double* h_u_out, double* h_phi_out, double* h_diag);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+long long accLB_launch_count(const accLB_ctx* ctx);
+
+/* Per-kernel device timing.  accLB_profile(ctx, 1) makes every later launch be bracketed by two CUDA events on
+ * the context's stream; accLB_profile_read synchronises the stream, adds the elapsed milliseconds and launch
+ * counts per kernel kind into ms[k], count[k] for k < min(n, ACCLB_NKERNELS) (HOST pointers) and clears the
+ * record.  Kinds: 0 k_normal, 1 k_lb (the fused LB step), 2 k_allen_cahn, 3 k_init, 4 k_moments,
+ * 5 k_diagnostics.  This is how bench.py measures the dominant kernel's duration inside the timed region. */
+#define ACCLB_NKERNELS 6
+int accLB_profile(accLB_ctx* ctx, int enable);
+int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
+
+/* Select the kernel variant of the LB update: 0 = default (best measured), other values are documented in
+ * DESIGN.md section 7 and exist so that bench.py / ncu can compare variants on identical inputs.  Results are
+ * identical to rounding for every variant.  ACCLB_EINVAL for an unknown variant. */
+int accLB_set_variant(accLB_ctx* ctx, int variant);
+
+/* Free the context (host memory only; the workspace stays the caller's). */
+int accLB_destroy(accLB_ctx* ctx);
+
+/* Text of the last error on this thread ("" if none).  The pointer stays valid until the next call. */
+const char* accLB_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ACCLB_H */

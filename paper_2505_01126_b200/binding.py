@@ -1,0 +1,189 @@
+"""Thin ctypes binding of ``libacclb.so`` (include/acclb.h): argument marshalling only.
+
+Every step of the path runs in the hand-written sm_100a kernels of ``csrc/``; PyTorch provides device memory
+(the workspace block and the field tensors) and the stream.  There is no CPU fallback: ``load()`` raises when
+the library is missing and every call needs a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libacclb.so"
+HEADER = _PKG.parent / "include" / "acclb.h"
+
+NDIAG = 9
+NKERNELS = 6
+KERNEL_NAMES = ("k_normal", "k_lb", "k_allen_cahn", "k_init", "k_moments", "k_diagnostics")
+DIAG_NAMES = ("ke", "dissipation", "sum_phi", "sum_pstar", "sum_mx", "sum_my", "sum_mz", "umax", "step")
+ERRORS = {0: "ACCLB_OK", -1: "ACCLB_EINVAL", -2: "ACCLB_EWORKSPACE", -3: "ACCLB_ECUDA", -4: "ACCLB_ENUMERIC"}
+
+SYMBOLS = ("accLB_workspace_bytes", "accLB_create", "accLB_init", "accLB_step", "accLB_moments",
+           "accLB_diagnostics", "accLB_run_host", "accLB_launch_count", "accLB_profile",
+           "accLB_profile_read", "accLB_set_variant", "accLB_destroy",
+           "accLB_last_error")
+
+
+class Params(C.Structure):
+    """Mirror of ``accLB_params``."""
+    _fields_ = [
+        ("tau", C.c_double),
+        ("two_phase", C.c_int),
+        ("rho_l", C.c_double), ("rho_g", C.c_double),
+        ("sigma", C.c_double), ("mobility", C.c_double), ("width", C.c_double),
+        ("force_type", C.c_int), ("force_amp", C.c_double), ("force_k", C.c_int),
+        ("store_fp32", C.c_int), ("host_staging", C.c_int),
+        ("device", C.c_int), ("stream", C.c_void_p),
+    ]
+
+
+class AccLBError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"{ERRORS.get(code, code)}: {text}")
+        self.code = code
+
+
+_lib = None
+_dp = C.c_void_p  # raw device / host addresses
+
+
+def load():
+    """dlopen libacclb.so; raise (never fall back) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2505_01126_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(str(LIB_PATH))
+    L.accLB_workspace_bytes.restype = C.c_size_t
+    L.accLB_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(Params)]
+    L.accLB_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.POINTER(Params), C.c_void_p, C.c_size_t]
+    L.accLB_init.argtypes = [C.c_void_p, _dp, _dp, _dp]
+    L.accLB_step.argtypes = [C.c_void_p, C.c_int]
+    L.accLB_moments.argtypes = [C.c_void_p, _dp, _dp, _dp]
+    L.accLB_diagnostics.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.c_int]
+    L.accLB_run_host.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, C.POINTER(C.c_double)]
+    L.accLB_launch_count.restype = C.c_longlong
+    L.accLB_launch_count.argtypes = [C.c_void_p]
+    L.accLB_profile.argtypes = [C.c_void_p, C.c_int]
+    L.accLB_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
+    L.accLB_set_variant.argtypes = [C.c_void_p, C.c_int]
+    L.accLB_destroy.argtypes = [C.c_void_p]
+    L.accLB_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(code):
+    if code != 0:
+        raise AccLBError(code, load().accLB_last_error().decode())
+
+
+def make_params(*, tau, two_phase=0, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0, width=4.0, force_type=0,
+                force_amp=0.0, force_k=1, store_fp32=0, host_staging=0, device=0, stream=None):
+    return Params(tau, int(two_phase), rho_l, rho_g, sigma, mobility, width, int(force_type), force_amp, int(force_k),
+                  int(store_fp32), int(host_staging), int(device), stream)
+
+
+def workspace_bytes(nx, ny, nz, params):
+    return load().accLB_workspace_bytes(nx, ny, nz, C.byref(params))
+
+
+class AccLB:
+    """One periodic box on one GPU.  Fields are fp64 CUDA tensors: scalars [nz][ny][nx], vectors [3][nz][ny][nx]."""
+
+    def __init__(self, nx, ny, nz, *, device=0, stream=None, **params):
+        import torch
+
+        L = load()
+        self._torch = torch
+        self.device = torch.device("cuda", device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        self.params = make_params(device=device, stream=stream.cuda_stream, **params)
+        self.shape = (nz, ny, nx)
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.n = nx * ny * nz
+        self.two_phase = bool(self.params.two_phase)
+        nbytes = L.accLB_workspace_bytes(nx, ny, nz, C.byref(self.params))
+        if nbytes == 0:
+            raise AccLBError(-1, f"invalid grid {nx}x{ny}x{nz} or parameters")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)  # torch owns device memory
+        self.workspace_bytes = nbytes
+        h = C.c_void_p()
+        _check(L.accLB_create(C.byref(h), nx, ny, nz, C.byref(self.params), self.workspace.data_ptr(), nbytes))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load().accLB_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev(self, t, shape):
+        torch = self._torch
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == tuple(shape), \
+            (t.device, t.dtype, tuple(t.shape), shape)
+        return t.data_ptr()
+
+    def init(self, rho, u, phi=None):
+        _check(load().accLB_init(self._h, self._dev(rho, self.shape), self._dev(u, (3,) + self.shape),
+                                 self._dev(phi, self.shape) if phi is not None else None))
+
+    def step(self, nsteps=1):
+        _check(load().accLB_step(self._h, int(nsteps)))
+
+    def moments(self, rho=None, u=None, phi=None):
+        torch = self._torch
+        kw = dict(dtype=torch.float64, device=self.device)
+        rho = torch.empty(self.shape, **kw) if rho is None else rho
+        u = torch.empty((3,) + self.shape, **kw) if u is None else u
+        if self.two_phase and phi is None:
+            phi = torch.empty(self.shape, **kw)
+        _check(load().accLB_moments(self._h, self._dev(rho, self.shape), self._dev(u, (3,) + self.shape),
+                                    self._dev(phi, self.shape) if self.two_phase else None))
+        return rho, u, (phi if self.two_phase else None)
+
+    def diagnostics(self):
+        out = (C.c_double * NDIAG)()
+        _check(load().accLB_diagnostics(self._h, out, NDIAG))
+        return dict(zip(DIAG_NAMES, list(out)))
+
+    def run_host(self, rho, u, phi, nsteps, rho_out=None, u_out=None, phi_out=None, diag=True):
+        """Host-buffer path: CPU tensors (pinned for asynchronous copies) in and out."""
+        def hp(t, shape):
+            if t is None:
+                return None
+            assert (not t.is_cuda) and t.dtype == self._torch.float64 and t.is_contiguous() and tuple(t.shape) == tuple(shape)
+            return t.data_ptr()
+        d = (C.c_double * NDIAG)() if diag else None
+        _check(load().accLB_run_host(self._h, hp(rho, self.shape), hp(u, (3,) + self.shape), hp(phi, self.shape),
+                                     int(nsteps), hp(rho_out, self.shape), hp(u_out, (3,) + self.shape),
+                                     hp(phi_out, self.shape), d))
+        return dict(zip(DIAG_NAMES, list(d))) if diag else None
+
+    def profile(self, enable=True):
+        _check(load().accLB_profile(self._h, int(bool(enable))))
+
+    def profile_read(self):
+        """{kernel: (total ms, launches)} since the last read; synchronises."""
+        ms = (C.c_double * NKERNELS)()
+        cnt = (C.c_longlong * NKERNELS)()
+        _check(load().accLB_profile_read(self._h, ms, cnt, NKERNELS))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(KERNEL_NAMES)}
+
+    def set_variant(self, v):
+        _check(load().accLB_set_variant(self._h, int(v)))
+
+    @property
+    def launch_count(self):
+        return int(load().accLB_launch_count(self._h))

@@ -1,0 +1,793 @@
+// libacclb.so -- kernels and C ABI (include/acclb.h) of the accLB per-time-step lattice update on sm_100a.
+//
+// Written from /root/reference/PAPER.md (arXiv 2505.01126).  One step (rows a1-a8):
+//   k_normal   (two-phase)  n = grad phi / (|grad phi| + 1e-12)                       PAPER.md:L61, L104, R17
+//   k_lb                    pull-stream (a1) -> moments (a2) -> geometry/forces (a3,a4) -> u (a5) ->
+//                           Hermite coefficient (a6) -> regularized reconstruction + aligned store (a7)
+//                                                                                     PAPER.md:L75-92 (Eqs. 4-7)
+//   k_allen_cahn (two-phase) conservative Allen-Cahn, flux-form WENO5 + lattice stencils, forward Euler (a8)
+//                                                                                     PAPER.md:L61-67 (Eq. 3)
+// State: post-collision, not yet streamed populations f*_i(x) in SoA [i][z][y][x], double-buffered (A/B), so the
+// pull f_i(x,t) = f*_i(x - c_i, t-1) reads shifted rows and every store is aligned; phi double-buffered.
+// No CPU fallback, no library kernels: everything the path computes runs in the kernels of this file.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/acclb.h"
+#include "d3q27.cuh"
+#include "stencils.cuh"
+
+namespace acclb {
+
+// ------------------------------------------------------------------------------------------------ parameters
+struct KP {
+  Grid G;
+  double omega, one_m_omega;  // 1/tau, 1 - 1/tau
+  double rho_g, drho;         // rho = rho_g + drho phi
+  double sig15w;              // gamma * 3 delta / 2                    PAPER.md:L102 + R8
+  double visc_pref;           // nu omega / cs2 = (tau - 1/2)/tau       PAPER.md:L104 (R9)
+  int ratio_ne;               // rho_l != rho_g
+  double D, kappa;            // D, 4 D / delta
+  int force_type;
+  double force_amp;
+  double nu, eps_pref;        // nu, nu / (2 cs4 tau^2) (R21)
+};
+
+// population storage: fp64, or fp32 deviation from the lattice weight (R22)
+template <typename ST> struct Pop;
+template <> struct Pop<double> {
+  static __device__ __forceinline__ double load(const double* p, int) { return __ldcs(p); }
+  static __device__ __forceinline__ void store(double* p, int, double v) { __stcs(p, v); }
+};
+template <> struct Pop<float> {
+  static __device__ __forceinline__ double load(const float* p, int i) { return (double)__ldcs(p) + w_of(i); }
+  static __device__ __forceinline__ void store(float* p, int i, double v) { __stcs(p, (float)(v - w_of(i))); }
+};
+
+__device__ __forceinline__ bool node_of_thread(const Grid& G, unsigned& k, int& x, int& y, int& z) {
+  k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= G.n) return false;
+  x = (int)(k % (unsigned)G.nx);
+  const unsigned yz = k / (unsigned)G.nx;
+  y = (int)(yz % (unsigned)G.ny);
+  z = (int)(yz / (unsigned)G.ny);
+  return true;
+}
+
+// R20 body-force density from the per-axis tables tabs = [sin kx x | cos kx x | sin ky y | cos ky y | sin kz z | cos kz z]
+__device__ __forceinline__ void body_force(const KP& P, const double* __restrict__ tabs, int x, int y, int z,
+                                           double (&Fb)[3]) {
+  Fb[0] = Fb[1] = Fb[2] = 0.0;
+  if (P.force_type == 0) return;
+  const double* sx = tabs;
+  const double* cx = sx + P.G.nx;
+  const double* sy = cx + P.G.nx;
+  const double* cy = sy + P.G.ny;
+  const double* sz = cy + P.G.ny;
+  const double* cz = sz + P.G.nz;
+  if (P.force_type == 1) {  // ABC
+    Fb[0] = P.force_amp * (__ldg(sz + z) + __ldg(cy + y));
+    Fb[1] = P.force_amp * (__ldg(sx + x) + __ldg(cz + z));
+    Fb[2] = P.force_amp * (__ldg(sy + y) + __ldg(cx + x));
+  } else {  // sine variant of BASELINE config 2
+    Fb[0] = P.force_amp * __ldg(sy + y);
+    Fb[1] = P.force_amp * __ldg(sz + z);
+    Fb[2] = P.force_amp * __ldg(sx + x);
+  }
+}
+
+// a1: pull-stream.  f_i(x,t) = f*_i(x - c_i, t-1), periodic wrap.   PAPER.md:L75/L85 (LHS of Eqs. 4, 6), L118
+template <typename ST>
+__device__ __forceinline__ void pull27(const ST* __restrict__ fin, const Grid& G, const Nbr& nb, double (&f)[Q]) {
+#pragma unroll
+  for (int i = 0; i < Q; ++i)
+    f[i] = Pop<ST>::load(fin + (size_t)i * G.n + nb.at(-cz_of(i), -cy_of(i), -cx_of(i)), i);
+}
+
+// a3-a5: interface geometry, total force, acceleration A = F / rho (R3) and density at a node.
+//   g = grad phi, kappa_c = div n (lattice stencils), rho = rho_g + drho phi (L102)
+//   F^s = -gamma (3 delta/2) kappa_c |g| g (L102, R8);  F^p = -p* cs2 grad rho (L102);
+//   F^nu = -((tau-1/2)/tau) (Pi - p* cs2 I - ut ut) . grad rho (L104, R9), ut = m + (F^s+F^p+F^b)/(2 rho);
+//   F = F^s + F^p + F^nu + F^b (Eq. 8).
+template <bool TWO_PHASE>
+__device__ __forceinline__ void node_accel(const KP& P, const double* __restrict__ phi, const double* __restrict__ nrm,
+                                           const double* __restrict__ tabs, const Nbr& nb, int x, int y, int z,
+                                           const Moments& M, bool with_visc, double (&A)[3], double& rho) {
+  double Fb[3];
+  body_force(P, tabs, x, y, z, Fb);
+  if (!TWO_PHASE) {
+    rho = 1.0;
+    A[0] = Fb[0]; A[1] = Fb[1]; A[2] = Fb[2];
+    return;
+  }
+  const unsigned n = P.G.n;
+  double g[3];
+  g[0] = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
+  g[1] = lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
+  g[2] = lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
+  const double kc = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(nrm + nb.at(dz, dy, dx)); }) +
+                    lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(nrm + n + nb.at(dz, dy, dx)); }) +
+                    lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(nrm + 2u * n + nb.at(dz, dy, dx)); });
+  const double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
+  rho = P.rho_g + P.drho * __ldg(phi + nb.at(0, 0, 0));
+  const double fs = -P.sig15w * kc * gn;
+  const double fp = -M.p * (1.0 / 3.0) * P.drho;
+  double F[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) F[a] = fs * g[a] + fp * g[a] + Fb[a];
+  if (with_visc && P.ratio_ne) {
+    const double h = 0.5 / rho;
+    const double ut[3] = {M.m[0] + F[0] * h, M.m[1] + F[1] * h, M.m[2] + F[2] * h};
+    const double dr[3] = {P.drho * g[0], P.drho * g[1], P.drho * g[2]};
+    const double p3 = M.p * (1.0 / 3.0);
+    const double sxx = M.Pi[0] - p3 - ut[0] * ut[0], syy = M.Pi[1] - p3 - ut[1] * ut[1], szz = M.Pi[2] - p3 - ut[2] * ut[2];
+    const double sxy = M.Pi[3] - ut[0] * ut[1], sxz = M.Pi[4] - ut[0] * ut[2], syz = M.Pi[5] - ut[1] * ut[2];
+    F[0] -= P.visc_pref * (sxx * dr[0] + sxy * dr[1] + sxz * dr[2]);
+    F[1] -= P.visc_pref * (sxy * dr[0] + syy * dr[1] + syz * dr[2]);
+    F[2] -= P.visc_pref * (sxz * dr[0] + syz * dr[1] + szz * dr[2]);
+  }
+  const double ir = 1.0 / rho;
+  A[0] = F[0] * ir; A[1] = F[1] * ir; A[2] = F[2] * ir;
+}
+
+// a6: a_ab = sum_i (f_i - f_i^eq + S_i/2) H_i,ab (Eq. 7) in closed form (O5'):
+//   sum f H = Pi - cs2 p* I,  sum f^eq H = uu,  sum S H = uA + Au.
+__device__ __forceinline__ void hermite_coeff(const Moments& M, const double (&u)[3], const double (&A)[3],
+                                              double (&a)[6]) {
+  const double p3 = M.p * (1.0 / 3.0);
+  a[0] = M.Pi[0] - p3 - u[0] * u[0] + u[0] * A[0];
+  a[1] = M.Pi[1] - p3 - u[1] * u[1] + u[1] * A[1];
+  a[2] = M.Pi[2] - p3 - u[2] * u[2] + u[2] * A[2];
+  a[3] = M.Pi[3] - u[0] * u[1] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
+  a[4] = M.Pi[4] - u[0] * u[2] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
+  a[5] = M.Pi[5] - u[1] * u[2] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
+}
+
+// ------------------------------------------------------------------------------------------------ kernels
+
+// Interface normal n = g / (|g| + 1e-12), g = grad phi by the lattice stencil.   PAPER.md:L61, L104; R17
+__global__ void __launch_bounds__(256) k_normal(KP P, const double* __restrict__ phi, double* __restrict__ nrm) {
+  unsigned k; int x, y, z;
+  if (!node_of_thread(P.G, k, x, y, z)) return;
+  Nbr nb;
+  make_nbr(P.G, x, y, z, nb);
+  double v[3][3][3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) v[a][b][c] = __ldg(phi + nb.row[a][b] + nb.x[c]);
+  double g[3];
+  gradient27(v, g);
+  const double inv = 1.0 / (sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]) + 1e-12);
+  nrm[k] = g[0] * inv;
+  nrm[P.G.n + k] = g[1] * inv;
+  nrm[2u * P.G.n + k] = g[2] * inv;
+}
+
+// The fused LB step, one node per thread (variant 1: scalar 64-bit accesses).
+template <typename ST, bool TWO_PHASE>
+__global__ void __launch_bounds__(128) k_lb(KP P, const ST* __restrict__ fin, ST* __restrict__ fout,
+                                            const double* __restrict__ phi, const double* __restrict__ nrm,
+                                            double* __restrict__ uout, const double* __restrict__ tabs) {
+  unsigned k; int x, y, z;
+  if (!node_of_thread(P.G, k, x, y, z)) return;
+  Nbr nb;
+  make_nbr(P.G, x, y, z, nb);
+  double f[Q];
+  pull27<ST>(fin, P.G, nb, f);
+  Moments M;
+  moments_of(f, M);
+  double A[3], rho;
+  node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, true, A, rho);
+  const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
+  if (TWO_PHASE) {
+    uout[k] = u[0];
+    uout[P.G.n + k] = u[1];
+    uout[2u * P.G.n + k] = u[2];
+  }
+  double a[6];
+  hermite_coeff(M, u, A, a);
+  // a7: Eq. 6 as one second-order Hermite-space population (see hermite2_populations)
+  const double U[3] = {u[0] + 0.5 * A[0], u[1] + 0.5 * A[1], u[2] + 0.5 * A[2]};
+  double T[6];
+  T[0] = u[0] * u[0] + P.one_m_omega * a[0] + u[0] * A[0];
+  T[1] = u[1] * u[1] + P.one_m_omega * a[1] + u[1] * A[1];
+  T[2] = u[2] * u[2] + P.one_m_omega * a[2] + u[2] * A[2];
+  T[3] = u[0] * u[1] + P.one_m_omega * a[3] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
+  T[4] = u[0] * u[2] + P.one_m_omega * a[4] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
+  T[5] = u[1] * u[2] + P.one_m_omega * a[5] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
+  hermite2_populations(M.p, U, T, f);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) Pop<ST>::store(fout + (size_t)i * P.G.n + k, i, f[i]);
+}
+
+// a8: conservative Allen-Cahn update (Eq. 3), forward Euler (R13):
+//   phi+ = phi - sum_e (Phi_e(x) - Phi_e(x - e)) + D lap phi - kappa div(phi (1 - phi) n),
+//   Phi_e = u_f WENO5(phi) in flux form (R12), lap / div by the lattice stencils.
+__global__ void __launch_bounds__(128) k_allen_cahn(KP P, const double* __restrict__ phi, const double* __restrict__ nrm,
+                                                    const double* __restrict__ u, double* __restrict__ phi_new) {
+  unsigned k; int x, y, z;
+  if (!node_of_thread(P.G, k, x, y, z)) return;
+  const Grid& G = P.G;
+  Nbr nb;
+  make_nbr(G, x, y, z, nb);
+  const unsigned n = G.n;
+  double v[3][3][3], pq[3][3][3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const double ph = __ldg(phi + nb.row[a][b] + nb.x[c]);
+        v[a][b][c] = ph;
+        pq[a][b][c] = ph * (1.0 - ph);
+      }
+  const double lap = laplacian27(v);
+  const double divq =
+      lattice_derivative<0>([&](int dz, int dy, int dx) { return pq[dz + 1][dy + 1][dx + 1] * __ldg(nrm + nb.at(dz, dy, dx)); }) +
+      lattice_derivative<1>([&](int dz, int dy, int dx) { return pq[dz + 1][dy + 1][dx + 1] * __ldg(nrm + n + nb.at(dz, dy, dx)); }) +
+      lattice_derivative<2>([&](int dz, int dy, int dx) { return pq[dz + 1][dy + 1][dx + 1] * __ldg(nrm + 2u * n + nb.at(dz, dy, dx)); });
+
+  double adv = 0.0;
+  {  // x faces
+    const unsigned r = nb.row[1][1];
+    const double pm3 = __ldg(phi + r + wrap_add(x, -3, G.nx)), pm2 = __ldg(phi + r + wrap_add(x, -2, G.nx));
+    const double pp2 = __ldg(phi + r + wrap_add(x, 2, G.nx)), pp3 = __ldg(phi + r + wrap_add(x, 3, G.nx));
+    const double um = __ldg(u + nb.at(0, 0, -1)), u0 = __ldg(u + k), up = __ldg(u + nb.at(0, 0, 1));
+    adv += face_flux(u0, up, pm2, v[1][1][0], v[1][1][1], v[1][1][2], pp2, pp3) -
+           face_flux(um, u0, pm3, pm2, v[1][1][0], v[1][1][1], v[1][1][2], pp2);
+  }
+  {  // y faces
+    const unsigned rz = (unsigned)z * (unsigned)G.ny;
+    auto at = [&](int kk) { return (rz + (unsigned)wrap_add(y, kk, G.ny)) * (unsigned)G.nx + (unsigned)x; };
+    const double pm3 = __ldg(phi + at(-3)), pm2 = __ldg(phi + at(-2)), pp2 = __ldg(phi + at(2)), pp3 = __ldg(phi + at(3));
+    const double* uy = u + n;
+    const double um = __ldg(uy + nb.at(0, -1, 0)), u0 = __ldg(uy + k), up = __ldg(uy + nb.at(0, 1, 0));
+    adv += face_flux(u0, up, pm2, v[1][0][1], v[1][1][1], v[1][2][1], pp2, pp3) -
+           face_flux(um, u0, pm3, pm2, v[1][0][1], v[1][1][1], v[1][2][1], pp2);
+  }
+  {  // z faces
+    auto at = [&](int kk) { return ((unsigned)wrap_add(z, kk, G.nz) * (unsigned)G.ny + (unsigned)y) * (unsigned)G.nx + (unsigned)x; };
+    const double pm3 = __ldg(phi + at(-3)), pm2 = __ldg(phi + at(-2)), pp2 = __ldg(phi + at(2)), pp3 = __ldg(phi + at(3));
+    const double* uz = u + 2u * n;
+    const double um = __ldg(uz + nb.at(-1, 0, 0)), u0 = __ldg(uz + k), up = __ldg(uz + nb.at(1, 0, 0));
+    adv += face_flux(u0, up, pm2, v[0][1][1], v[1][1][1], v[2][1][1], pp2, pp3) -
+           face_flux(um, u0, pm3, pm2, v[0][1][1], v[1][1][1], v[2][1][1], pp2);
+  }
+  phi_new[k] = v[1][1][1] + (-adv + P.D * lap - P.kappa * divq);
+}
+
+// Initial populations (R15): f_i(x,0) = f_i^eq(p*,u0) - S_i(u0,A)/2 with A from F^s + F^p + F^b (F^nu := 0),
+// written "pushed" to x - c_i so that the first pull returns them at x.
+template <typename ST, bool TWO_PHASE>
+__global__ void __launch_bounds__(128) k_init(KP P, const double* __restrict__ rho_in, const double* __restrict__ u_in,
+                                              const double* __restrict__ phi, const double* __restrict__ nrm,
+                                              const double* __restrict__ tabs, ST* __restrict__ fout) {
+  unsigned k; int x, y, z;
+  if (!node_of_thread(P.G, k, x, y, z)) return;
+  Nbr nb;
+  make_nbr(P.G, x, y, z, nb);
+  Moments M;
+  M.p = rho_in[k];
+  M.m[0] = M.m[1] = M.m[2] = 0.0;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) M.Pi[j] = 0.0;
+  double A[3], rho;
+  node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, false, A, rho);
+  const double u[3] = {u_in[k], u_in[P.G.n + k], u_in[2u * P.G.n + k]};
+  const double U[3] = {u[0] - 0.5 * A[0], u[1] - 0.5 * A[1], u[2] - 0.5 * A[2]};
+  double T[6];
+  T[0] = u[0] * u[0] - u[0] * A[0];
+  T[1] = u[1] * u[1] - u[1] * A[1];
+  T[2] = u[2] * u[2] - u[2] * A[2];
+  T[3] = u[0] * u[1] - 0.5 * (u[0] * A[1] + u[1] * A[0]);
+  T[4] = u[0] * u[2] - 0.5 * (u[0] * A[2] + u[2] * A[0]);
+  T[5] = u[1] * u[2] - 0.5 * (u[1] * A[2] + u[2] * A[1]);
+  double f[Q];
+  hermite2_populations(M.p, U, T, f);
+#pragma unroll
+  for (int i = 0; i < Q; ++i)
+    Pop<ST>::store(fout + (size_t)i * P.G.n + nb.at(-cz_of(i), -cy_of(i), -cx_of(i)), i, f[i]);
+}
+
+// a9: (p*, u) of the current state; the state is unchanged.
+template <typename ST, bool TWO_PHASE>
+__global__ void __launch_bounds__(128) k_moments(KP P, const ST* __restrict__ fin, const double* __restrict__ phi,
+                                                 const double* __restrict__ nrm, const double* __restrict__ tabs,
+                                                 double* __restrict__ rho_out, double* __restrict__ u_out) {
+  unsigned k; int x, y, z;
+  if (!node_of_thread(P.G, k, x, y, z)) return;
+  Nbr nb;
+  make_nbr(P.G, x, y, z, nb);
+  double f[Q];
+  pull27<ST>(fin, P.G, nb, f);
+  Moments M;
+  moments_of(f, M);
+  double A[3], rho;
+  node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, true, A, rho);
+  if (rho_out) rho_out[k] = M.p;
+  if (u_out) {
+    u_out[k] = M.m[0] + 0.5 * A[0];
+    u_out[P.G.n + k] = M.m[1] + 0.5 * A[1];
+    u_out[2u * P.G.n + k] = M.m[2] + 0.5 * A[2];
+  }
+}
+
+// a9: diagnostics (R21).  acc[0..6] += sum (rho |u|^2/2, eps, phi, p*, m_x, m_y, m_z); acc[7] = max |u| (as ordered
+// bits).  Grid-stride; per-thread partials -> warp shuffle -> one atomic per block and quantity.
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+constexpr int DIAG_THREADS = 128;
+
+template <typename ST, bool TWO_PHASE>
+__global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __restrict__ fin,
+                                                              const double* __restrict__ phi,
+                                                              const double* __restrict__ nrm,
+                                                              const double* __restrict__ tabs, double* __restrict__ acc) {
+  double s[7] = {0, 0, 0, 0, 0, 0, 0};
+  double umax = 0.0;
+  const Grid& G = P.G;
+  for (unsigned k = blockIdx.x * blockDim.x + threadIdx.x; k < G.n; k += gridDim.x * blockDim.x) {
+    const int x = (int)(k % (unsigned)G.nx);
+    const unsigned yz = k / (unsigned)G.nx;
+    const int y = (int)(yz % (unsigned)G.ny), z = (int)(yz / (unsigned)G.ny);
+    Nbr nb;
+    make_nbr(G, x, y, z, nb);
+    double f[Q];
+    pull27<ST>(fin, G, nb, f);
+    Moments M;
+    moments_of(f, M);
+    double A[3], rho;
+    node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, true, A, rho);
+    const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};
+    double a[6];
+    hermite_coeff(M, u, A, a);
+    const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    const double aa = a[0] * a[0] + a[1] * a[1] + a[2] * a[2] + 2.0 * (a[3] * a[3] + a[4] * a[4] + a[5] * a[5]);
+    s[0] += 0.5 * rho * uu;
+    s[1] += P.eps_pref * aa;
+    if (TWO_PHASE) s[2] += __ldg(phi + k);
+    s[3] += M.p;
+    s[4] += M.m[0];
+    s[5] += M.m[1];
+    s[6] += M.m[2];
+    umax = fmax(umax, sqrt(uu));
+  }
+  __shared__ double sh[8][DIAG_THREADS / 32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int j = 0; j < 7; ++j) {
+    const double r = warp_sum(s[j]);
+    if (lane == 0) sh[j][wid] = r;
+  }
+  {
+    const double r = warp_max(umax);
+    if (lane == 0) sh[7][wid] = r;
+  }
+  __syncthreads();
+  if (threadIdx.x < 8) {
+    const int j = threadIdx.x;
+    double r = sh[j][0];
+    for (int w = 1; w < DIAG_THREADS / 32; ++w) r = (j < 7) ? r + sh[j][w] : fmax(r, sh[j][w]);
+    if (j < 7) atomicAdd(acc + j, r);
+    else atomicMax(reinterpret_cast<unsigned long long*>(acc + 7), (unsigned long long)__double_as_longlong(r));  // r >= 0
+  }
+}
+
+}  // namespace acclb
+
+// ================================================================================================== host / ABI
+using namespace acclb;
+
+struct accLB_ctx {
+  accLB_params prm;
+  KP kp;
+  int nx, ny, nz;
+  size_t n;
+  cudaStream_t stream;
+  // carved from the caller's workspace
+  void* f[2];
+  double* phi[2];
+  double* u;
+  double* nrm;
+  double* tabs;
+  double* acc;
+  double* stage;  // [5 n] rho | u(3) | phi, host_staging only
+  int cur;        // f[cur], phi[cur] hold the current state
+  long long step;
+  long long launches;
+  int variant;
+  int profiling;
+  struct Rec { int kind; cudaEvent_t e0, e1; };
+  std::vector<Rec> recs;
+};
+
+// Counts a kernel launch and, when profiling is on, brackets it with two events on the context's stream.
+struct LaunchScope {
+  accLB_ctx* s;
+  accLB_ctx::Rec r;
+  bool on;
+  LaunchScope(accLB_ctx* s_, int kind) : s(s_), on(s_->profiling != 0) {
+    r.kind = kind;
+    if (on) {
+      on = cudaEventCreate(&r.e0) == cudaSuccess && cudaEventCreate(&r.e1) == cudaSuccess;
+      if (on) cudaEventRecord(r.e0, s->stream);
+    }
+  }
+  ~LaunchScope() {
+    s->launches++;
+    if (on) {
+      cudaEventRecord(r.e1, s->stream);
+      s->recs.push_back(r);
+    }
+  }
+};
+enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5 };
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+static size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
+  if (!p) return false;
+  if (nx < 4 || ny < 4 || nz < 4 || (nx & 1)) return false;
+  if ((double)nx * (double)ny * (double)nz >= 2147483648.0) return false;
+  if (!(p->tau > 0.5) || !std::isfinite(p->tau)) return false;
+  if (p->force_type < 0 || p->force_type > 2) return false;
+  if (p->two_phase) {
+    if (!(p->rho_l > 0.0) || !(p->rho_g > 0.0) || !(p->width > 0.0) || !(p->mobility >= 0.0)) return false;
+  }
+  return true;
+}
+
+struct Carve {
+  size_t f, phi, u, nrm, tabs, acc, stage, total;
+};
+static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
+  const size_t n = (size_t)nx * ny * nz;
+  Carve c;
+  c.f = align256(27 * n * (p->store_fp32 ? 4 : 8));
+  c.phi = p->two_phase ? align256(n * 8) : 0;
+  c.u = p->two_phase ? align256(3 * n * 8) : 0;
+  c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
+  c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
+  c.acc = align256(16 * 8);
+  c.stage = p->host_staging ? align256(5 * n * 8) : 0;
+  c.total = 2 * c.f + 2 * c.phi + c.u + c.nrm + c.tabs + c.acc + c.stage;
+  return c;
+}
+
+#define CK(call)                                                                                      \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) return fail(ACCLB_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+extern "C" {
+
+size_t accLB_workspace_bytes(int nx, int ny, int nz, const accLB_params* p) {
+  if (!valid_args(nx, ny, nz, p)) return 0;
+  return carve(nx, ny, nz, p).total;
+}
+
+int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p, void* workspace,
+                 size_t workspace_bytes) {
+  if (!out) return fail(ACCLB_EINVAL, "accLB_create: out is NULL");
+  *out = nullptr;
+  if (!valid_args(nx, ny, nz, p))
+    return fail(ACCLB_EINVAL, "accLB_create: invalid grid %dx%dx%d or parameters (need nx,ny,nz >= 4, nx even, "
+                              "nodes < 2^31, tau > 0.5, force_type in 0..2, two_phase: rho_l, rho_g, width > 0)",
+                nx, ny, nz);
+  const Carve c = carve(nx, ny, nz, p);
+  if (!workspace || ((size_t)workspace & 255)) return fail(ACCLB_EWORKSPACE, "accLB_create: workspace NULL or not 256-byte aligned");
+  if (workspace_bytes < c.total)
+    return fail(ACCLB_EWORKSPACE, "accLB_create: workspace of %zu bytes, need %zu", workspace_bytes, c.total);
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (p->device < 0 || p->device >= ndev) return fail(ACCLB_EINVAL, "accLB_create: device %d of %d", p->device, ndev);
+  CK(cudaSetDevice(p->device));
+
+  accLB_ctx* s = new (std::nothrow) accLB_ctx();
+  if (!s) return fail(ACCLB_EINVAL, "accLB_create: out of host memory");
+  s->prm = *p;
+  s->nx = nx; s->ny = ny; s->nz = nz;
+  s->n = (size_t)nx * ny * nz;
+  s->stream = (cudaStream_t)p->stream;
+  char* w = (char*)workspace;
+  s->f[0] = w; w += c.f;
+  s->f[1] = w; w += c.f;
+  s->phi[0] = p->two_phase ? (double*)w : nullptr; w += c.phi;
+  s->phi[1] = p->two_phase ? (double*)w : nullptr; w += c.phi;
+  s->u = p->two_phase ? (double*)w : nullptr; w += c.u;
+  s->nrm = p->two_phase ? (double*)w : nullptr; w += c.nrm;
+  s->tabs = (double*)w; w += c.tabs;
+  s->acc = (double*)w; w += c.acc;
+  s->stage = p->host_staging ? (double*)w : nullptr; w += c.stage;
+  s->cur = 0; s->step = 0; s->launches = 0; s->variant = 0; s->profiling = 0;
+
+  KP& k = s->kp;
+  k.G.nx = nx; k.G.ny = ny; k.G.nz = nz; k.G.n = (unsigned)s->n;
+  k.omega = 1.0 / p->tau;
+  k.one_m_omega = 1.0 - k.omega;
+  k.rho_g = p->two_phase ? p->rho_g : 1.0;
+  k.drho = p->two_phase ? p->rho_l - p->rho_g : 0.0;
+  k.sig15w = p->sigma * (1.5 * p->width);
+  k.visc_pref = (p->tau - 0.5) / p->tau;
+  k.ratio_ne = p->two_phase && p->rho_l != p->rho_g;
+  k.D = p->mobility;
+  k.kappa = p->two_phase ? 4.0 * p->mobility / p->width : 0.0;
+  k.force_type = p->force_type;
+  k.force_amp = p->force_amp;
+  k.nu = (p->tau - 0.5) / 3.0;
+  k.eps_pref = k.nu / (2.0 * (1.0 / 9.0) * p->tau * p->tau);
+
+  // R20: per-axis sin/cos tables, libm on the host, k = 2 pi force_k / N, integer node coordinates
+  std::vector<double> t((size_t)2 * (nx + ny + nz));
+  const double two_pi = 6.283185307179586476925286766559;
+  const int dims[3] = {nx, ny, nz};
+  size_t o = 0;
+  for (int ax = 0; ax < 3; ++ax) {
+    const double kk = two_pi * p->force_k / dims[ax];
+    for (int j = 0; j < dims[ax]; ++j) t[o + j] = sin(kk * (double)j);
+    for (int j = 0; j < dims[ax]; ++j) t[o + dims[ax] + j] = cos(kk * (double)j);
+    o += (size_t)2 * dims[ax];
+  }
+  cudaError_t e = cudaMemcpyAsync(s->tabs, t.data(), t.size() * 8, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e != cudaSuccess) {
+    delete s;
+    return fail(ACCLB_ECUDA, "accLB_create: table upload: %s", cudaGetErrorString(e));
+  }
+  *out = s;
+  g_err[0] = 0;
+  return ACCLB_OK;
+}
+
+static int launch_normal(accLB_ctx* s) {
+  {
+    LaunchScope ls(s, KIND_NORMAL);
+    k_normal<<<blocks_for(s->n, 256), 256, 0, s->stream>>>(s->kp, s->phi[s->cur], s->nrm);
+  }
+  CK(cudaGetLastError());
+  return ACCLB_OK;
+}
+
+int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* phi) {
+  if (!s || !rho || !u) return fail(ACCLB_EINVAL, "accLB_init: NULL argument");
+  if (s->prm.two_phase && !phi) return fail(ACCLB_EINVAL, "accLB_init: phi is NULL for a two-phase context");
+  CK(cudaSetDevice(s->prm.device));
+  s->cur = 0;
+  s->step = 0;
+  const unsigned nb = blocks_for(s->n, 128);
+  if (s->prm.two_phase) {
+    CK(cudaMemcpyAsync(s->phi[0], phi, s->n * 8, cudaMemcpyDeviceToDevice, s->stream));
+    int r = launch_normal(s);
+    if (r) return r;
+    LaunchScope ls(s, KIND_INIT);
+    if (s->prm.store_fp32)
+      k_init<float, true><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, s->phi[0], s->nrm, s->tabs, (float*)s->f[0]);
+    else
+      k_init<double, true><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, s->phi[0], s->nrm, s->tabs, (double*)s->f[0]);
+  } else {
+    LaunchScope ls(s, KIND_INIT);
+    if (s->prm.store_fp32)
+      k_init<float, false><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, nullptr, nullptr, s->tabs, (float*)s->f[0]);
+    else
+      k_init<double, false><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, nullptr, nullptr, s->tabs, (double*)s->f[0]);
+  }
+  CK(cudaGetLastError());
+  return ACCLB_OK;
+}
+
+int accLB_step(accLB_ctx* s, int nsteps) {
+  if (!s || nsteps < 0) return fail(ACCLB_EINVAL, "accLB_step: NULL context or negative nsteps");
+  CK(cudaSetDevice(s->prm.device));
+  const unsigned nb = blocks_for(s->n, 128);
+  for (int it = 0; it < nsteps; ++it) {
+    const int c = s->cur, d = c ^ 1;
+    if (s->prm.two_phase) {
+      int r = launch_normal(s);
+      if (r) return r;
+      {
+        LaunchScope ls(s, KIND_LB);
+        if (s->prm.store_fp32)
+          k_lb<float, true><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], (float*)s->f[d], s->phi[c], s->nrm, s->u, s->tabs);
+        else
+          k_lb<double, true><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], (double*)s->f[d], s->phi[c], s->nrm, s->u, s->tabs);
+      }
+      {
+        LaunchScope ls(s, KIND_AC);
+        k_allen_cahn<<<nb, 128, 0, s->stream>>>(s->kp, s->phi[c], s->nrm, s->u, s->phi[d]);
+      }
+    } else {
+      LaunchScope ls(s, KIND_LB);
+      if (s->prm.store_fp32)
+        k_lb<float, false><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], (float*)s->f[d], nullptr, nullptr, nullptr, s->tabs);
+      else
+        k_lb<double, false><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], (double*)s->f[d], nullptr, nullptr, nullptr, s->tabs);
+    }
+    s->cur = d;
+    s->step += 1;
+  }
+  CK(cudaGetLastError());
+  return ACCLB_OK;
+}
+
+int accLB_moments(accLB_ctx* s, double* rho, double* u, double* phi) {
+  if (!s) return fail(ACCLB_EINVAL, "accLB_moments: NULL context");
+  CK(cudaSetDevice(s->prm.device));
+  const unsigned nb = blocks_for(s->n, 128);
+  const int c = s->cur;
+  if (s->prm.two_phase) {
+    int r = launch_normal(s);
+    if (r) return r;
+    {
+      LaunchScope ls(s, KIND_MOMENTS);
+      if (s->prm.store_fp32)
+        k_moments<float, true><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], s->phi[c], s->nrm, s->tabs, rho, u);
+      else
+        k_moments<double, true><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], s->phi[c], s->nrm, s->tabs, rho, u);
+    }
+    if (phi) CK(cudaMemcpyAsync(phi, s->phi[c], s->n * 8, cudaMemcpyDeviceToDevice, s->stream));
+  } else {
+    LaunchScope ls(s, KIND_MOMENTS);
+    if (s->prm.store_fp32)
+      k_moments<float, false><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], nullptr, nullptr, s->tabs, rho, u);
+    else
+      k_moments<double, false><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], nullptr, nullptr, s->tabs, rho, u);
+  }
+  CK(cudaGetLastError());
+  return ACCLB_OK;
+}
+
+int accLB_diagnostics(accLB_ctx* s, double* out, int n_out) {
+  if (!s || !out || n_out < ACCLB_NDIAG) return fail(ACCLB_EINVAL, "accLB_diagnostics: NULL argument or n_out < %d", ACCLB_NDIAG);
+  CK(cudaSetDevice(s->prm.device));
+  const int c = s->cur;
+  CK(cudaMemsetAsync(s->acc, 0, 16 * 8, s->stream));
+  unsigned nb = blocks_for(s->n, DIAG_THREADS);
+  const unsigned cap = 148u * 16u;  // a multiple of the SM count; grid-stride beyond that
+  if (nb > cap) nb = cap;
+  if (s->prm.two_phase) {
+    int r = launch_normal(s);
+    if (r) return r;
+    LaunchScope ls(s, KIND_DIAG);
+    if (s->prm.store_fp32)
+      k_diagnostics<float, true><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const float*)s->f[c], s->phi[c], s->nrm, s->tabs, s->acc);
+    else
+      k_diagnostics<double, true><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const double*)s->f[c], s->phi[c], s->nrm, s->tabs, s->acc);
+  } else {
+    LaunchScope ls(s, KIND_DIAG);
+    if (s->prm.store_fp32)
+      k_diagnostics<float, false><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const float*)s->f[c], nullptr, nullptr, s->tabs, s->acc);
+    else
+      k_diagnostics<double, false><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const double*)s->f[c], nullptr, nullptr, s->tabs, s->acc);
+  }
+  CK(cudaGetLastError());
+  double h[8];
+  CK(cudaMemcpyAsync(h, s->acc, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  const double inv_n = 1.0 / (double)s->n;
+  out[0] = h[0] * inv_n;
+  out[1] = h[1] * inv_n;
+  out[2] = h[2];
+  out[3] = h[3];
+  out[4] = h[4];
+  out[5] = h[5];
+  out[6] = h[6];
+  out[7] = h[7];
+  out[8] = (double)s->step;
+  for (int j = 0; j < 8; ++j)
+    if (!std::isfinite(out[j])) return fail(ACCLB_ENUMERIC, "accLB_diagnostics: entry %d is not finite", j);
+  return ACCLB_OK;
+}
+
+int accLB_run_host(accLB_ctx* s, const double* h_rho, const double* h_u, const double* h_phi, int nsteps,
+                   double* h_rho_out, double* h_u_out, double* h_phi_out, double* h_diag) {
+  if (!s || !h_rho || !h_u || nsteps < 0) return fail(ACCLB_EINVAL, "accLB_run_host: NULL argument or negative nsteps");
+  if (!s->stage) return fail(ACCLB_EINVAL, "accLB_run_host: context was created without host_staging");
+  if (s->prm.two_phase && !h_phi) return fail(ACCLB_EINVAL, "accLB_run_host: h_phi is NULL for a two-phase context");
+  CK(cudaSetDevice(s->prm.device));
+  const size_t n = s->n;
+  double* d_rho = s->stage;
+  double* d_u = s->stage + n;
+  double* d_phi = s->stage + 4 * n;
+  CK(cudaMemcpyAsync(d_rho, h_rho, n * 8, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(d_u, h_u, 3 * n * 8, cudaMemcpyHostToDevice, s->stream));
+  if (s->prm.two_phase) CK(cudaMemcpyAsync(d_phi, h_phi, n * 8, cudaMemcpyHostToDevice, s->stream));
+  int r = accLB_init(s, d_rho, d_u, s->prm.two_phase ? d_phi : nullptr);
+  if (r) return r;
+  r = accLB_step(s, nsteps);
+  if (r) return r;
+  if (h_rho_out || h_u_out || h_phi_out) {
+    r = accLB_moments(s, d_rho, d_u, d_phi);
+    if (r) return r;
+    if (h_rho_out) CK(cudaMemcpyAsync(h_rho_out, d_rho, n * 8, cudaMemcpyDeviceToHost, s->stream));
+    if (h_u_out) CK(cudaMemcpyAsync(h_u_out, d_u, 3 * n * 8, cudaMemcpyDeviceToHost, s->stream));
+    if (h_phi_out && s->prm.two_phase) CK(cudaMemcpyAsync(h_phi_out, d_phi, n * 8, cudaMemcpyDeviceToHost, s->stream));
+  }
+  if (h_diag) {
+    r = accLB_diagnostics(s, h_diag, ACCLB_NDIAG);
+    if (r) return r;
+  }
+  CK(cudaStreamSynchronize(s->stream));
+  return ACCLB_OK;
+}
+
+long long accLB_launch_count(const accLB_ctx* s) { return s ? s->launches : 0; }
+
+int accLB_set_variant(accLB_ctx* s, int variant) {
+  if (!s) return fail(ACCLB_EINVAL, "accLB_set_variant: NULL context");
+  if (variant < 0 || variant > 1) return fail(ACCLB_EINVAL, "accLB_set_variant: unknown variant %d", variant);
+  s->variant = variant;
+  return ACCLB_OK;
+}
+
+static void drop_records(accLB_ctx* s) {
+  for (auto& r : s->recs) {
+    cudaEventDestroy(r.e0);
+    cudaEventDestroy(r.e1);
+  }
+  s->recs.clear();
+}
+
+int accLB_profile(accLB_ctx* s, int enable) {
+  if (!s) return fail(ACCLB_EINVAL, "accLB_profile: NULL context");
+  s->profiling = enable != 0;
+  return ACCLB_OK;
+}
+
+int accLB_profile_read(accLB_ctx* s, double* ms, long long* count, int n) {
+  if (!s || !ms || !count || n < 1) return fail(ACCLB_EINVAL, "accLB_profile_read: NULL argument");
+  CK(cudaSetDevice(s->prm.device));
+  CK(cudaStreamSynchronize(s->stream));
+  for (auto& r : s->recs) {
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, r.e0, r.e1));
+    if (r.kind < n && r.kind < ACCLB_NKERNELS) {
+      ms[r.kind] += (double)t;
+      count[r.kind] += 1;
+    }
+  }
+  drop_records(s);
+  return ACCLB_OK;
+}
+
+int accLB_destroy(accLB_ctx* s) {
+  if (!s) return fail(ACCLB_EINVAL, "accLB_destroy: NULL context");
+  drop_records(s);
+  delete s;
+  return ACCLB_OK;
+}
+
+const char* accLB_last_error(void) { return g_err; }
+
+}  // extern "C"

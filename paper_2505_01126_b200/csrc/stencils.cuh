@@ -1,0 +1,128 @@
+// Periodic neighbour indexing, the lattice-stencil derivative operators of PAPER.md:L104 and the WENO5 face
+// reconstruction of PAPER.md:L67 (Jiang-Shu, R12), device side.  Part of the CUDA product path.
+//
+// The D3Q27 weights factorise, w_i = o(cx) o(cy) o(cz) with o(0) = 2/3, o(+-1) = 1/6, so the stencils
+//   d_a Psi  = (1/cs2) sum_i w_i c_ia Psi(x + c_i)
+//   lap Psi  = (2/cs2) sum_i w_i (Psi(x + c_i) - Psi(x))        PAPER.md:L104 as repaired by R7
+// are evaluated in separable form: a central difference along a, smoothed with (1,4,1)/6 along the two other
+// axes.  Same numbers as the 27-term sums up to rounding order.
+#pragma once
+
+namespace acclb {
+
+struct Grid {
+  int nx, ny, nz;
+  unsigned n;  // nodes; n < 2^31 (checked at create)
+};
+
+// Wrapped coordinates of the 3x3x3 neighbourhood of a node: periodic boundaries as in-kernel index wrap
+// (compare-select, no modulo), replacing the paper's halo exchange.
+struct Nbr {
+  int x[3];            // x-1, x, x+1 wrapped
+  unsigned row[3][3];  // [dz+1][dy+1] -> (zz * ny + yy) * nx
+  __device__ __forceinline__ unsigned at(int dz, int dy, int dx) const { return row[dz + 1][dy + 1] + x[dx + 1]; }
+};
+
+__device__ __forceinline__ int wrap_dec(int a, int n) { return a == 0 ? n - 1 : a - 1; }
+__device__ __forceinline__ int wrap_inc(int a, int n) { return a == n - 1 ? 0 : a + 1; }
+// a + k for |k| <= 3 on a period n >= 4
+__device__ __forceinline__ int wrap_add(int a, int k, int n) {
+  int r = a + k;
+  if (r < 0) r += n;
+  if (r >= n) r -= n;
+  return r;
+}
+
+__device__ __forceinline__ void make_nbr(const Grid& G, int x, int y, int z, Nbr& nb) {
+  nb.x[0] = wrap_dec(x, G.nx); nb.x[1] = x; nb.x[2] = wrap_inc(x, G.nx);
+  const int ys[3] = {wrap_dec(y, G.ny), y, wrap_inc(y, G.ny)};
+  const int zs[3] = {wrap_dec(z, G.nz), z, wrap_inc(z, G.nz)};
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) nb.row[a][b] = ((unsigned)zs[a] * (unsigned)G.ny + (unsigned)ys[b]) * (unsigned)G.nx;
+}
+
+// Lattice derivative along AX of a periodic field given through `val(dz, dy, dx)`.
+//   (1/cs2) sum_i w_i c_i,AX val(c_i) = (1/72) sum_{p,q in -1..1} W(p) W(q) (val(+1; p,q) - val(-1; p,q)), W = (1,4,1)
+template <int AX, class V>
+__device__ __forceinline__ double lattice_derivative(V val) {
+  double acc = 0.0;
+#pragma unroll
+  for (int p = -1; p <= 1; ++p)
+#pragma unroll
+    for (int q = -1; q <= 1; ++q) {
+      const double wgt = (p == 0 ? 4.0 : 1.0) * (q == 0 ? 4.0 : 1.0);
+      double d;
+      if (AX == 0) d = val(p, q, 1) - val(p, q, -1);        // (dz,dy) = (p,q)
+      else if (AX == 1) d = val(p, 1, q) - val(p, -1, q);   // (dz,dx) = (p,q)
+      else d = val(1, p, q) - val(-1, p, q);                // (dy,dx) = (p,q)
+      acc = fma(wgt, d, acc);
+    }
+  return acc * (1.0 / 72.0);
+}
+
+// Gradient and Laplacian of one scalar whose 27 neighbourhood values are in v[dz+1][dy+1][dx+1].
+__device__ __forceinline__ void gradient27(const double (&v)[3][3][3], double (&g)[3]) {
+  g[0] = lattice_derivative<0>([&](int dz, int dy, int dx) { return v[dz + 1][dy + 1][dx + 1]; });
+  g[1] = lattice_derivative<1>([&](int dz, int dy, int dx) { return v[dz + 1][dy + 1][dx + 1]; });
+  g[2] = lattice_derivative<2>([&](int dz, int dy, int dx) { return v[dz + 1][dy + 1][dx + 1]; });
+}
+
+__device__ __forceinline__ double laplacian27(const double (&v)[3][3][3]) {
+  // (2/cs2) sum_i w_i (v_i - v_0) = 6 (sum_i w_i v_i - v_0), w_i = W W W / 216
+  double acc = 0.0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+      const double row = v[a][b][0] + 4.0 * v[a][b][1] + v[a][b][2];
+      acc = fma((a == 1 ? 4.0 : 1.0) * (b == 1 ? 4.0 : 1.0), row, acc);
+    }
+  return 6.0 * (acc * (1.0 / 216.0) - v[1][1][1]);
+}
+
+// Jiang-Shu WENO5 value at the face downwind of `c`, from the five upwind-ordered cell values (R12;
+// PAPER.md:L67, ref. [19]): candidates q_k, smoothness b_k, weights d_k / (eps + b_k)^2, d = (.1,.6,.3), eps = 1e-6.
+// The three weight divisions and the normalisation are folded into one division by multiplying through with
+// the product of the (eps + b_k)^2.  Every operation is an explicitly rounded intrinsic so that the two cells
+// sharing a face evaluate bit-identical fluxes (exact conservation of sum phi, R12).
+__device__ __forceinline__ double weno5_face(double a, double b, double c, double d, double e) {
+  const double k1312 = 13.0 / 12.0, sixth = 1.0 / 6.0, eps = 1e-6;
+  const double q0 = __dmul_rn(__fma_rn(11.0, c, __fma_rn(-7.0, b, __dmul_rn(2.0, a))), sixth);
+  const double q1 = __dmul_rn(__fma_rn(2.0, d, __fma_rn(5.0, c, -b)), sixth);
+  const double q2 = __dmul_rn(__fma_rn(5.0, d, __fma_rn(2.0, c, -e)), sixth);
+  const double s0 = __dadd_rn(__fma_rn(-2.0, b, a), c);          // a - 2b + c
+  const double t0 = __fma_rn(3.0, c, __fma_rn(-4.0, b, a));      // a - 4b + 3c
+  const double s1 = __dadd_rn(__fma_rn(-2.0, c, b), d);          // b - 2c + d
+  const double t1 = __dsub_rn(b, d);                             // b - d
+  const double s2 = __dadd_rn(__fma_rn(-2.0, d, c), e);          // c - 2d + e
+  const double t2 = __dadd_rn(__fma_rn(-4.0, d, __dmul_rn(3.0, c)), e);  // 3c - 4d + e
+  const double b0 = __fma_rn(k1312, __dmul_rn(s0, s0), __dmul_rn(0.25, __dmul_rn(t0, t0)));
+  const double b1 = __fma_rn(k1312, __dmul_rn(s1, s1), __dmul_rn(0.25, __dmul_rn(t1, t1)));
+  const double b2 = __fma_rn(k1312, __dmul_rn(s2, s2), __dmul_rn(0.25, __dmul_rn(t2, t2)));
+  const double r0 = __dadd_rn(eps, b0), r1 = __dadd_rn(eps, b1), r2 = __dadd_rn(eps, b2);
+  const double e0 = __dmul_rn(r0, r0), e1 = __dmul_rn(r1, r1), e2 = __dmul_rn(r2, r2);
+  const double n0 = __dmul_rn(0.1, __dmul_rn(e1, e2));
+  const double n1 = __dmul_rn(0.6, __dmul_rn(e0, e2));
+  const double n2 = __dmul_rn(0.3, __dmul_rn(e0, e1));
+  const double num = __fma_rn(n2, q2, __fma_rn(n1, q1, __dmul_rn(n0, q0)));
+  const double den = __dadd_rn(__dadd_rn(n0, n1), n2);
+  return __ddiv_rn(num, den);
+}
+
+// Advective flux through the face between cells L and R = L + e: u_f = (u_L + u_R)/2, upwinded by its sign
+// (R12, R29).  pm2..pp3 are phi at L-2, L-1, L, L+1 (= R), L+2, L+3.
+__device__ __forceinline__ double face_flux(double uL, double uR, double pm2, double pm1, double p0, double pp1,
+                                            double pp2, double pp3) {
+  const double uf = __dmul_rn(0.5, __dadd_rn(uL, uR));
+  const bool pos = uf >= 0.0;
+  const double a = pos ? pm2 : pp3;
+  const double b = pos ? pm1 : pp2;
+  const double c = pos ? p0 : pp1;
+  const double d = pos ? pp1 : p0;
+  const double e = pos ? pp2 : pm1;
+  return __dmul_rn(uf, weno5_face(a, b, c, d, e));
+}
+
+}  // namespace acclb

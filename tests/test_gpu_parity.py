@@ -1,0 +1,263 @@
+"""GPU-vs-oracle parity through the C ABI (the first gate).  Same seeded inputs on both sides; compared element by
+element on the ABI-level fields p* ("rho"), u, phi and on the diagnostics.  Tolerances are BASELINE.json's:
+fp64 max|d| <= 1e-11 after 100 steps (smooth cases) / after each of the first 10 steps (turbulent cases);
+conserved sums 1e-12 relative; fp32 population storage: relative L2 <= 1e-5.  Why 1e-11 is safe: DESIGN.md section 4.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2505_01126_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def gpu_sim(acclb, cfg, shape=None, **extra):
+    n = cfg["n"]
+    nx, ny, nz = shape or (n, n, n)
+    sim = acclb.AccLB(nx, ny, nz, **cfg["params"], **extra)
+    dev = sim.device
+    rho = torch.from_numpy(np.ascontiguousarray(cfg["rho"])).to(dev)
+    u = torch.from_numpy(np.ascontiguousarray(cfg["u"])).to(dev)
+    phi = torch.from_numpy(np.ascontiguousarray(cfg["phi"])).to(dev) if cfg["phi"] is not None else None
+    sim.init(rho, u, phi)
+    return sim
+
+
+def cpu_sim(cfg, shape=None):
+    n = cfg["n"]
+    nx, ny, nz = shape or (n, n, n)
+    o = oracle.Oracle(nx, ny, nz, **cfg["params"])
+    o.init(cfg["rho"], cfg["u"], cfg["phi"])
+    return o
+
+
+def max_diffs(sim, o):
+    r, u, p = sim.moments()
+    ro, uo, po = o.moments()
+    d = {"rho": np.abs(r.cpu().numpy() - ro).max(), "u": np.abs(u.cpu().numpy() - uo).max()}
+    if po is not None:
+        d["phi"] = np.abs(p.cpu().numpy() - po).max()
+    return d
+
+
+def assert_parity(sim, o, tol=TOL, what=""):
+    d = max_diffs(sim, o)
+    assert all(v <= tol for v in d.values()), (what, d)
+    return d
+
+
+def crop(cfg, shape):
+    """Cut a config's cubic fields down to a ragged box (nx, ny, nz); the fields stay smooth only in the interior,
+    which is fine: parity does not need smoothness."""
+    nx, ny, nz = shape
+    out = dict(cfg)
+    out["rho"] = np.ascontiguousarray(cfg["rho"][:nz, :ny, :nx])
+    out["u"] = np.ascontiguousarray(cfg["u"][:, :nz, :ny, :nx])
+    out["phi"] = None if cfg["phi"] is None else np.ascontiguousarray(cfg["phi"][:nz, :ny, :nx])
+    return out
+
+
+# ---------------------------------------------------------------------------------------------- config 1
+def test_config1_tgv_100_steps(acclb):
+    cfg = wl.make_config("tgv")
+    sim, o = gpu_sim(acclb, cfg), cpu_sim(cfg)
+    assert_parity(sim, o, what="t=0")
+    sim.step(100)
+    o.step(100)
+    assert_parity(sim, o, what="t=100")
+    dg, do = sim.diagnostics(), o.diagnostics()
+    assert dg["step"] == 100
+    for k in ("ke", "dissipation", "sum_pstar"):
+        assert abs(dg[k] - do[k]) <= 1e-12 * abs(do[k]), (k, dg[k], do[k])
+    for k in ("sum_mx", "sum_my", "sum_mz"):
+        assert abs(dg[k] - do[k]) <= 1e-12
+    assert abs(dg["umax"] - do["umax"]) <= 1e-13
+    # the closed form the oracle is pinned to (P6) holds for the GPU path as well
+    nu, k2 = (0.8 - 0.5) / 3.0, 3.0 * (2 * np.pi / 32) ** 2
+    assert abs(dg["dissipation"] / (2 * nu * k2 * dg["ke"]) - 1.0) < 0.02
+
+
+# ---------------------------------------------------------------------------------------------- config 2
+def test_config2_hit_first_10_steps_and_conserved_sums(acclb):
+    cfg = wl.make_config("hit", n=64)
+    sim, o = gpu_sim(acclb, cfg), cpu_sim(cfg)
+    for t in range(10):
+        sim.step(1)
+        o.step(1)
+        assert_parity(sim, o, what=f"t={t + 1}")
+    d0 = sim.diagnostics()
+    sim.step(490)
+    d1 = sim.diagnostics()
+    n3 = 64 ** 3
+    assert abs(d1["sum_pstar"] - d0["sum_pstar"]) <= 1e-12 * n3
+    for k in ("sum_mx", "sum_my", "sum_mz"):  # sum of the sine forcing is zero (R20)
+        assert abs(d1[k] - d0[k]) <= 1e-12 * n3 * 0.03
+    assert np.isfinite(d1["ke"]) and 0.1 < d1["ke"] / d0["ke"] < 1.5
+
+
+def test_config2_abc_forcing_ragged_box(acclb):
+    """Ragged non-cubic box (several blocks + a tail in every kernel), ABC forcing."""
+    cfg = crop(wl.make_config("hit", n=48), (44, 30, 18))
+    cfg["params"].update(force_type=1, force_amp=2e-5, force_k=2, tau=0.6)
+    sim, o = gpu_sim(acclb, cfg, shape=(44, 30, 18)), cpu_sim(cfg, shape=(44, 30, 18))
+    sim.step(10)
+    o.step(10)
+    assert_parity(sim, o)
+
+
+# ---------------------------------------------------------------------------------------------- config 3
+@pytest.mark.parametrize("ratio", [1.0, 10.0])
+def test_config3_droplet_100_steps(acclb, ratio):
+    cfg = wl.make_config("droplet", n=48, density_ratio=ratio)
+    sim, o = gpu_sim(acclb, cfg), cpu_sim(cfg)
+    assert_parity(sim, o, what="t=0")
+    sim.step(100)
+    o.step(100)
+    assert_parity(sim, o, what="t=100")
+    dg, do = sim.diagnostics(), o.diagnostics()
+    assert abs(dg["sum_phi"] - do["sum_phi"]) <= 1e-12 * do["sum_phi"]
+    assert abs(dg["sum_pstar"] - do["sum_pstar"]) <= 1e-12 * 48 ** 3
+    assert abs(dg["ke"] - do["ke"]) <= 1e-11 * max(do["ke"], 1e-30) + 1e-22
+
+
+def test_config3_sum_phi_conserved_long_run(acclb):
+    cfg = wl.make_config("droplet", n=64)
+    sim = gpu_sim(acclb, cfg)
+    s0 = sim.diagnostics()["sum_phi"]
+    sim.step(1000)
+    d = sim.diagnostics()
+    assert abs(d["sum_phi"] - s0) <= 1e-12 * s0
+    assert d["umax"] < 1e-3
+
+
+# ---------------------------------------------------------------------------------------------- config 4
+def test_config4_bubbly_first_10_steps(acclb):
+    cfg = wl.make_config("bubbly", n=64, void_fraction=0.03)
+    sim, o = gpu_sim(acclb, cfg), cpu_sim(cfg)
+    for t in range(10):
+        sim.step(1)
+        o.step(1)
+        assert_parity(sim, o, what=f"t={t + 1}")
+    d0 = sim.diagnostics()
+    sim.step(190)
+    d1 = sim.diagnostics()
+    assert abs(d1["sum_phi"] - d0["sum_phi"]) <= 1e-12 * d0["sum_phi"]
+    assert abs(d1["sum_pstar"] - d0["sum_pstar"]) <= 1e-12 * 64 ** 3
+
+
+def test_two_phase_ragged_box_ratio10_with_forcing(acclb):
+    cfg = crop(wl.make_config("bubbly", n=48, void_fraction=0.05), (40, 26, 22))
+    cfg["params"].update(rho_l=10.0, rho_g=1.0, tau=0.7, force_type=1, force_amp=1e-5)
+    shape = (40, 26, 22)
+    sim, o = gpu_sim(acclb, cfg, shape=shape), cpu_sim(cfg, shape=shape)
+    sim.step(10)
+    o.step(10)
+    assert_parity(sim, o)
+
+
+def test_thin_slab_flat_interface(acclb):
+    """Smallest legal box (4 x 4 x 64): every stencil wraps onto itself; flat interface pair (P9 set-up)."""
+    nx, ny, nz = 4, 4, 64
+    z = np.arange(nz, dtype=np.float64)
+    prof = 0.5 * (np.tanh(2 * (z - 16) / 2.0) - np.tanh(2 * (z - 48) / 2.0))
+    cfg = dict(n=None, params=dict(tau=0.8, two_phase=1, rho_l=1.0, rho_g=1.0, sigma=0.01, mobility=0.05, width=4.0,
+                                   force_type=0, force_amp=0.0, force_k=1),
+               rho=np.ones((nz, ny, nx)), u=np.zeros((3, nz, ny, nx)),
+               phi=np.ascontiguousarray(np.broadcast_to(prof[:, None, None], (nz, ny, nx))))
+    sim, o = gpu_sim(acclb, cfg, shape=(nx, ny, nz)), cpu_sim(cfg, shape=(nx, ny, nz))
+    sim.step(50)
+    o.step(50)
+    assert_parity(sim, o)
+
+
+# ---------------------------------------------------------------------------------------------- fp32 storage
+def rel_l2(a, b):
+    return np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300)
+
+
+@pytest.mark.parametrize("name,n,steps,kw", [("tgv", 32, 100, {}), ("hit", 48, 10, {}),
+                                             ("bubbly", 48, 10, dict(void_fraction=0.03))])
+def test_fp32_population_storage(acclb, name, n, steps, kw):
+    cfg = wl.make_config(name, n=n, **kw)
+    sim, o = gpu_sim(acclb, cfg, store_fp32=1), cpu_sim(cfg)
+    sim.step(steps)
+    o.step(steps)
+    r, u, p = sim.moments()
+    ro, uo, po = o.moments()
+    assert rel_l2(r.cpu().numpy(), ro) <= 1e-5
+    assert rel_l2(u.cpu().numpy(), uo) <= 1e-5
+    if po is not None:
+        assert rel_l2(p.cpu().numpy(), po) <= 1e-5
+
+
+# ---------------------------------------------------------------------------------------------- API behaviour
+def test_moments_leave_state_unchanged_and_step_counts(acclb):
+    cfg = wl.make_config("bubbly", n=32, void_fraction=0.03)
+    a, b = gpu_sim(acclb, cfg), gpu_sim(acclb, cfg)
+    a.step(3)
+    a.moments()
+    a.diagnostics()
+    a.step(2)
+    b.step(5)
+    for x, y in zip(a.moments(), b.moments()):
+        assert torch.equal(x, y)
+    assert a.diagnostics()["step"] == 5
+    # re-init restarts the clock and reproduces the run bit for bit
+    first = [t.clone() for t in b.moments()]
+    dev = b.device
+    b.init(torch.from_numpy(cfg["rho"]).to(dev), torch.from_numpy(cfg["u"]).to(dev), torch.from_numpy(cfg["phi"]).to(dev))
+    assert b.diagnostics()["step"] == 0
+    b.step(5)
+    for x, y in zip(first, b.moments()):
+        assert torch.equal(x, y)
+
+
+def test_run_host_equals_device_path(acclb):
+    cfg = wl.make_config("bubbly", n=32, void_fraction=0.03)
+    sim = gpu_sim(acclb, cfg, host_staging=1)
+    sim.step(7)
+    ref = [t.cpu() for t in sim.moments()]
+    dref = sim.diagnostics()
+    n = 32
+    rho_o, u_o, phi_o = torch.empty(n, n, n, dtype=torch.float64), torch.empty(3, n, n, n, dtype=torch.float64), torch.empty(n, n, n, dtype=torch.float64)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    d = sim.run_host(pin(cfg["rho"]), pin(cfg["u"]), pin(cfg["phi"]), 7, rho_o, u_o, phi_o)
+    assert torch.equal(rho_o, ref[0]) and torch.equal(u_o, ref[1]) and torch.equal(phi_o, ref[2])
+    assert d["step"] == 7 and abs(d["sum_phi"] - dref["sum_phi"]) <= 1e-12 * dref["sum_phi"]
+    plain = gpu_sim(acclb, cfg)
+    with pytest.raises(acclb.AccLBError):
+        plain.run_host(pin(cfg["rho"]), pin(cfg["u"]), pin(cfg["phi"]), 1)
+
+
+def test_launch_count_and_errors(acclb):
+    cfg = wl.make_config("tgv")
+    sim = gpu_sim(acclb, cfg)
+    c0 = sim.launch_count
+    sim.step(4)
+    assert sim.launch_count - c0 == 4          # one fused kernel per single-phase step
+    cfg2 = wl.make_config("droplet", n=32)
+    sim2 = gpu_sim(acclb, cfg2)
+    c0 = sim2.launch_count
+    sim2.step(4)
+    assert sim2.launch_count - c0 == 12        # normal + LB + Allen-Cahn per two-phase step
+    with pytest.raises(acclb.AccLBError):
+        sim.step(-1)
+    with pytest.raises(acclb.AccLBError):
+        acclb.AccLB(31, 32, 32, tau=0.8)
+
+
+def test_non_default_stream(acclb):
+    cfg = wl.make_config("tgv")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        sim = gpu_sim(acclb, cfg)
+        sim.step(20)
+        got = [t.cpu() for t in sim.moments()[:2]]
+    ref = gpu_sim(acclb, cfg)
+    ref.step(20)
+    for x, y in zip(got, ref.moments()[:2]):
+        assert torch.equal(x, y.cpu())
