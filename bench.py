@@ -1,0 +1,425 @@
+#!/usr/bin/env python
+"""bench.py -- GLUPS of the accLB hot path on B200 (BASELINE.json metric) + roofline + CPU-oracle baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]              # this repo's CUDA path, ONE JSON line
+    python bench.py --impl reference [--steps K] [--warmup W]        # the CPU oracle as it stands, ONE JSON line
+    torchrun --nproc-per-node N ... bench.py --gpus N ...            # N independent replicas ("replicas only")
+    python bench.py --sweep [--sweep-out FILE]                       # BASELINE config 5 table (several JSON lines)
+
+A "step" is one pass of the whole hot path (rows a1-a8: pull-stream, moments, phase geometry,
+forces, velocity, Hermite coefficient, regularized reconstruction, conservative Allen-Cahn update) over one lattice.
+Workload at N = 1: BASELINE config 4 (bubble-laden forced turbulence, 512^3, fp64, two-phase), the configuration the
+north-star bar (>= 80 % of the HBM roofline at 512^3 fp64) is quoted on; inputs are seeded and synthetic
+(paper_2505_01126_b200/workloads.py).  `value` times accLB_step with the state resident in HBM; `e2e` times
+accLB_run_host (host buffers in, host buffers out, copies inside the timed region).  The state (66 GB) is far larger
+than L2 (126 MB), so no L2 flush is needed between iterations.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "GLUPS on 1 B200 (fp64) and achieved HBM GB/s as fraction of roofline"
+UNIT = "GLUPS"
+# Algorithmic bytes per lattice update (DESIGN.md section 7 / SURVEY.md 8(d)):
+#   fused LB kernel: 27 populations read + 27 written, 8 B (fp64) or 4 B (fp32 storage) each;
+#   whole two-phase step: + phi read + phi written (8 B each).
+def lb_bytes_per_lup(fp32):
+    return 54 * (4 if fp32 else 8)
+
+
+def step_bytes_per_lup(fp32, two_phase):
+    return lb_bytes_per_lup(fp32) + (16 if two_phase else 0)
+
+
+def hbm_peak():
+    """(GB/s, 'measured'|'fallback'): MEASURED_PEAKS.json hbm_gbs, else the profiling guide's fallback 6650."""
+    p = ROOT / "MEASURED_PEAKS.json"
+    try:
+        return float(json.loads(p.read_text())["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, smax, power, reasons = [], 0.0, [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                smax = max(smax, float(f[1]))
+                power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": smax, "reasons": sorted(reasons), "samples": len(sm),
+                "power_w_max": max(power) if power else None}
+
+
+# ------------------------------------------------------------------------------------------------------ workload
+WORKLOADS = {  # bench name -> (workloads.make_config name, description)
+    "bubbly": ("bubbly", "BASELINE config 4: bubble-laden forced turbulence, two-phase, tau=0.505, 60 bubbles R=16 at 512^3"),
+    "hit": ("hit", "BASELINE config 2 setup: single-phase forced isotropic turbulence, tau=0.51"),
+    "sweep1": ("sweep1", "BASELINE config 5 single-phase (config 2 setup)"),
+    "sweep2": ("sweep2", "BASELINE config 5 two-phase (config 4 setup at 3 % void fraction)"),
+}
+
+
+def make_workload(name, n):
+    from paper_2505_01126_b200 import workloads as wl
+
+    return wl.make_config(WORKLOADS[name][0], n=n)
+
+
+# ------------------------------------------------------------------------------------------------------ oracle leg
+def oracle_threads():
+    return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+
+
+def oracle_sample(cfg, s):
+    """Periodic s^3 sub-box at the origin of the workload's fields, and the oracle set up on it (forcing keeps the
+    period of the full box).  A bounded sample of the same workload: same parameters, same value distributions."""
+    import oracle
+    from paper_2505_01126_b200 import workloads as wl
+
+    n = cfg["n"]
+    s = min(s, n)
+    rho = wl.subbox(cfg["rho"], (0, 0, 0), s)
+    u = wl.subbox(cfg["u"], (0, 0, 0), s)
+    phi = wl.subbox(cfg["phi"], (0, 0, 0), s) if cfg["phi"] is not None else None
+    o = oracle.Oracle(s, s, s, **cfg["params"], force_period=(n, n, n), force_origin=(0, 0, 0))
+    o.init(rho, u, phi)
+    return o, s
+
+
+def time_oracle(cfg, steps, warmup, budget_s):
+    """Time the oracle as it stands on a sub-box sized so that (steps + warmup) steps take about budget_s.
+    Returns (GLUPS, seconds per step, sub-box edge, cores)."""
+    o, s0 = oracle_sample(cfg, 32)
+    o.step(1)
+    t = time.perf_counter()
+    o.step(2)
+    rate = 2 * s0 ** 3 / (time.perf_counter() - t)  # LUP/s, calibration only
+    o.close()
+    s = 32
+    for cand in (48, 64, 96, 128, 192, 256):
+        if cand <= cfg["n"] and (steps + warmup) * cand ** 3 / rate <= budget_s:
+            s = cand
+    o, s = oracle_sample(cfg, s)
+    o.step(warmup)
+    t = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t
+    d = o.diagnostics()
+    o.close()
+    assert d["step"] == steps + warmup
+    return s ** 3 * steps / dt / 1e9, dt / steps, s, oracle_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on this arm's config/metric/unit (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+
+    oracle.build()
+    cfg = make_workload(args.workload, args.n)
+    glups, sec, s, cores = time_oracle(cfg, args.steps, args.warmup, budget_s=150.0)
+    two_phase = bool(cfg["params"]["two_phase"])
+    sample = (f"{s}^3 periodic sub-box at the origin of the {args.n}^3 {args.workload} fields, {args.warmup} warm-up + "
+              f"{args.steps} timed oracle steps, gcc -O2 -fopenmp, {cores} threads")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": glups, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload} {args.n}^3 {'two' if two_phase else 'single'}-phase fp64 "
+                               f"(timed on a {s}^3 sub-box sample)", "n": args.n, "sample_n": s,
+                   "two_phase": two_phase},
+        "cpu_baseline": {"value": glups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": glups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------ CUDA arm
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=True, variant=None, barrier=None,
+                 sample_clocks=True):
+    """Time `steps` steps of the CUDA path on one GPU.  Returns a dict of raw measurements (this rank's)."""
+    import numpy as np
+    import torch
+    from paper_2505_01126_b200 import binding
+
+    n = cfg["n"]
+    two_phase = bool(cfg["params"]["two_phase"])
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    stream = torch.cuda.current_stream(dev)
+    sim = binding.AccLB(n, n, n, device=local_rank, stream=stream, store_fp32=int(fp32), host_staging=int(e2e),
+                        **cfg["params"])
+    if variant is not None:
+        sim.set_variant(variant)
+    h = {k: torch.from_numpy(np.ascontiguousarray(cfg[k])) for k in ("rho", "u", "phi") if cfg[k] is not None}
+    d = {k: v.to(dev) for k, v in h.items()}
+    sim.init(d["rho"], d["u"], d.get("phi"))
+    sim.step(warmup)
+    torch.cuda.synchronize(dev)
+    diag0 = sim.diagnostics()
+    sync = barrier or (lambda: None)
+
+    # ---- timed region: `steps` steps, state resident in HBM; per-kernel events on the launching stream
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.profile(True)
+    launches0 = sim.launch_count
+    sync()
+    torch.cuda.synchronize(dev)
+    with ClockSampler(local_rank) as clk:
+        ev0.record(stream)
+        sim.step(steps)
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        if not sample_clocks:
+            clk.lines.clear()
+    sync()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.launch_count - launches0
+    kernels = sim.profile_read()
+    sim.profile(False)
+    diag1 = sim.diagnostics()
+
+    out = {"ms": ms, "launches": launches, "kernels": kernels, "clocks": clk.summary(), "diag0": diag0, "diag1": diag1,
+           "workspace_bytes": sim.workspace_bytes, "n": n, "two_phase": two_phase}
+
+    # ---- end to end: HOST buffers in, HOST buffers out, through accLB_run_host (copies inside the timed region)
+    if e2e:
+        pin = {k: v.pin_memory() for k, v in h.items()}
+        res = {k: torch.empty_like(v).pin_memory() for k, v in h.items()}
+        sim.run_host(pin["rho"], pin["u"], pin.get("phi"), 1, res["rho"], res["u"], res.get("phi"), diag=True)  # warm-up
+        sync()
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        dg = sim.run_host(pin["rho"], pin["u"], pin.get("phi"), steps, res["rho"], res["u"], res.get("phi"), diag=True)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        wall = time.perf_counter() - t0
+        sync()
+        nbytes = sum(v.numel() * 8 for v in h.values())
+        out["e2e"] = {"ms": e0.elapsed_time(e1), "wall_ms": wall * 1e3, "h2d": nbytes, "d2h": nbytes + 9 * 8,
+                      "diag": dg}
+    sim.close()
+    del d
+    torch.cuda.empty_cache()
+    return out
+
+
+def roofline_of(meas, steps, fp32):
+    """Roofline object for the dominant kernel (the fused LB step k_lb), from its CUDA-event durations."""
+    n3 = meas["n"] ** 3
+    ms_lb, cnt_lb = meas["kernels"]["k_lb"]
+    peak, how = hbm_peak()
+    per_launch_ms = ms_lb / max(cnt_lb, 1)
+    achieved = lb_bytes_per_lup(fp32) * n3 / (per_launch_ms * 1e-3) / 1e9
+    total_ms = sum(v[0] for v in meas["kernels"].values())
+    r = {"bound": "hbm", "kernel": "k_lb", "achieved": achieved, "peak": peak, "peak_source": how, "unit": "GB/s",
+         "frac": achieved / peak, "traffic": None, "bytes_per_launch": lb_bytes_per_lup(fp32) * n3,
+         "kernel_ms_per_launch": per_launch_ms, "kernel_share_of_step": ms_lb / total_ms if total_ms else None,
+         "kernels_ms_per_step": {k: v[0] / steps for k, v in meas["kernels"].items() if v[1]},
+         "step_bytes_per_lup": step_bytes_per_lup(fp32, meas["two_phase"])}
+    r["step_achieved"] = r["step_bytes_per_lup"] * n3 * steps / (meas["ms"] * 1e-3) / 1e9
+    r["step_frac"] = r["step_achieved"] / peak
+    t = ROOT / "profiles" / "traffic.json"  # dram bytes per launch of k_lb from the committed ncu --set full capture
+    try:
+        tj = json.loads(t.read_text())
+        key = f"{'two' if meas['two_phase'] else 'single'}_{'fp32' if fp32 else 'fp64'}_{meas['n']}"
+        r["traffic"] = tj.get(key)
+    except Exception:
+        pass
+    return r
+
+
+def run_cuda(args):
+    import torch
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA arm has no CPU fallback)")
+    barrier = None
+    if world > 1:
+        import torch.distributed as dist
+
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+        def barrier():
+            dist.barrier()
+
+    from paper_2505_01126_b200 import build as _build
+
+    if rank == 0:
+        _build.build()
+    if barrier:
+        barrier()
+    cfg = make_workload(args.workload, args.n)
+    meas = measure_cuda(cfg, args.steps, args.warmup, local_rank=local_rank, world=world, fp32=bool(args.fp32),
+                        e2e=not args.no_e2e, variant=args.variant, barrier=barrier)
+    ms, e2e_ms = meas["ms"], meas.get("e2e", {}).get("ms", 0.0)
+    if world > 1:  # replicas only: every rank ran the same-sized independent problem; time = max over ranks
+        import torch.distributed as dist
+
+        t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=f"cuda:{local_rank}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = t.tolist()
+    if rank != 0:
+        if world > 1:
+            torch.distributed.destroy_process_group()
+        return
+    n3 = args.n ** 3
+    value = world * n3 * args.steps / (ms * 1e-3) / 1e9
+    two_phase = meas["two_phase"]
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload} {args.n}^3 {'two' if two_phase else 'single'}-phase, "
+                               f"{'fp32' if args.fp32 else 'fp64'} population storage, fp64 arithmetic; "
+                               + WORKLOADS[args.workload][1],
+                   "n": args.n, "two_phase": two_phase, "population_storage": "fp32" if args.fp32 else "fp64",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"state of {meas['workspace_bytes'] / 1e9:.1f} GB streams through a 126 MB L2 every step; no flush needed",
+                   "lups_per_step": world * n3},
+        "clocks": meas["clocks"],
+        "gpu_launches": meas["launches"],
+        "roofline": roofline_of(meas, args.steps, bool(args.fp32)),
+        "diagnostics": {"before": meas["diag0"], "after": meas["diag1"]},
+    }
+    if "e2e" in meas:
+        e = meas["e2e"]
+        line["e2e"] = {"value": world * n3 * args.steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+                       "h2d_bytes_per_step": e["h2d"] / args.steps, "d2h_bytes_per_step": e["d2h"] / args.steps,
+                       "h2d_bytes_per_call": e["h2d"], "d2h_bytes_per_call": e["d2h"], "ms_per_call": e2e_ms,
+                       "wall_ms_per_call": e["wall_ms"],
+                       "call": f"accLB_run_host(nsteps={args.steps}): pinned host p*,u,phi -> init -> steps -> moments + "
+                               "diagnostics -> pinned host"}
+    if world == 1 and not args.no_cpu:
+        import oracle
+
+        oracle.build()
+        glups, sec, s, cores = time_oracle(cfg, 5, 1, budget_s=20.0)
+        line["cpu_baseline"] = {"value": glups, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{s}^3 periodic sub-box at the origin of the same {args.n}^3 fields, 1 warm-up + "
+                                          f"5 timed oracle steps ({sec:.2f} s/step), gcc -O2 -fopenmp"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------------ config 5 sweep
+def run_sweep(args):
+    """BASELINE config 5: N in {64,...,512}, single- and two-phase, fp64 and fp32 population storage; 200 timed steps
+    after 20 warm-up steps unless --steps/--warmup say otherwise.  One JSON line per case (not the driver's line)."""
+    peak, how = hbm_peak()
+    sizes = [int(s) for s in args.sweep_sizes.split(",")]
+    rows = []
+    for name in ("sweep1", "sweep2"):
+        for n in sizes:
+            cfg = make_workload(name, n)
+            for fp32 in (False, True):
+                m = measure_cuda(cfg, args.steps, args.warmup, fp32=fp32, e2e=False, variant=args.variant,
+                                 sample_clocks=False)
+                glups = n ** 3 * args.steps / (m["ms"] * 1e-3) / 1e9
+                bpl = step_bytes_per_lup(fp32, m["two_phase"])
+                row = {"case": name, "n": n, "two_phase": m["two_phase"], "storage": "fp32" if fp32 else "fp64",
+                       "glups": glups, "ms_per_step": m["ms"] / args.steps, "bytes_per_lup": bpl,
+                       "gbs": glups * bpl, "frac_of_hbm_peak": glups * bpl / peak, "peak": peak, "peak_source": how,
+                       "kernels_ms_per_step": {k: v[0] / args.steps for k, v in m["kernels"].items() if v[1]}}
+                rows.append(row)
+                print(json.dumps(row), flush=True)
+    if args.sweep_out:
+        Path(args.sweep_out).parent.mkdir(parents=True, exist_ok=True)
+        Path(args.sweep_out).write_text("\n".join(json.dumps(r) for r in rows) + "\n")
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", choices=("cuda", "reference"), default="cuda")
+    ap.add_argument("--workload", choices=sorted(WORKLOADS), default="bubbly")
+    ap.add_argument("--n", type=int, default=512, help="grid edge (default: the 512^3 the metric is quoted on)")
+    ap.add_argument("--fp32", type=int, default=0, help="1: fp32 population storage (arithmetic stays fp64)")
+    ap.add_argument("--variant", type=int, default=None, help="kernel variant (accLB_set_variant), default = best")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--sweep-sizes", default="64,128,256,384,512")
+    ap.add_argument("--sweep-out", default=None)
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("bench.py: --steps >= 1 and --warmup >= 0")
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()
