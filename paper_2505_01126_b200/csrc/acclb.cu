@@ -90,32 +90,15 @@ __device__ __forceinline__ void pull27(const ST* __restrict__ fin, const Grid& G
     f[i] = Pop<ST>::load(fin + (size_t)i * G.n + nb.at(-cz_of(i), -cy_of(i), -cx_of(i)), i);
 }
 
-// a3-a5: interface geometry, total force, acceleration A = F / rho (R3) and density at a node.
-//   g = grad phi, kappa_c = div n (lattice stencils), rho = rho_g + drho phi (L102)
+// a4-a5: total force, acceleration A = F / rho (R3) and density at a node from its interface geometry.
+//   g = grad phi, gn = |g|, kc = kappa_c = div n, phi0 = phi(x);  rho = rho_g + drho phi
 //   F^s = -gamma (3 delta/2) kappa_c |g| g (L102, R8);  F^p = -p* cs2 grad rho (L102);
 //   F^nu = -((tau-1/2)/tau) (Pi - p* cs2 I - ut ut) . grad rho (L104, R9), ut = m + (F^s+F^p+F^b)/(2 rho);
 //   F = F^s + F^p + F^nu + F^b (Eq. 8).
-template <bool TWO_PHASE>
-__device__ __forceinline__ void node_accel(const KP& P, const double* __restrict__ phi, const double* __restrict__ nrm,
-                                           const double* __restrict__ tabs, const Nbr& nb, int x, int y, int z,
-                                           const Moments& M, bool with_visc, double (&A)[3], double& rho) {
-  double Fb[3];
-  body_force(P, tabs, x, y, z, Fb);
-  if (!TWO_PHASE) {
-    rho = 1.0;
-    A[0] = Fb[0]; A[1] = Fb[1]; A[2] = Fb[2];
-    return;
-  }
-  const unsigned n = P.G.n;
-  double g[3];
-  g[0] = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
-  g[1] = lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
-  g[2] = lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
-  const double kc = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(nrm + nb.at(dz, dy, dx)); }) +
-                    lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(nrm + n + nb.at(dz, dy, dx)); }) +
-                    lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(nrm + 2u * n + nb.at(dz, dy, dx)); });
-  const double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
-  rho = P.rho_g + P.drho * __ldg(phi + nb.at(0, 0, 0));
+__device__ __forceinline__ void accel_from_geometry(const KP& P, const Moments& M, const double (&g)[3], double gn,
+                                                    double kc, double phi0, const double (&Fb)[3], bool with_visc,
+                                                    double (&A)[3], double& rho) {
+  rho = P.rho_g + P.drho * phi0;
   const double fs = -P.sig15w * kc * gn;
   const double fp = -M.p * (1.0 / 3.0) * P.drho;
   double F[3];
@@ -136,6 +119,31 @@ __device__ __forceinline__ void node_accel(const KP& P, const double* __restrict
   A[0] = F[0] * ir; A[1] = F[1] * ir; A[2] = F[2] * ir;
 }
 
+// a3-a5 for the one-node-per-thread kernels: g = grad phi and kappa_c = div n by the lattice stencils
+// straight from global memory (phi, and the normal field written by k_normal), then the force.
+template <bool TWO_PHASE>
+__device__ __forceinline__ void node_accel(const KP& P, const double* __restrict__ phi, const double* __restrict__ nrm,
+                                           const double* __restrict__ tabs, const Nbr& nb, int x, int y, int z,
+                                           const Moments& M, bool with_visc, double (&A)[3], double& rho) {
+  double Fb[3];
+  body_force(P, tabs, x, y, z, Fb);
+  if (!TWO_PHASE) {
+    rho = 1.0;
+    A[0] = Fb[0]; A[1] = Fb[1]; A[2] = Fb[2];
+    return;
+  }
+  const unsigned n = P.G.n;
+  double g[3];
+  g[0] = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
+  g[1] = lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
+  g[2] = lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
+  const double kc = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(nrm + nb.at(dz, dy, dx)); }) +
+                    lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(nrm + n + nb.at(dz, dy, dx)); }) +
+                    lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(nrm + 2u * n + nb.at(dz, dy, dx)); });
+  const double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
+  accel_from_geometry(P, M, g, gn, kc, __ldg(phi + nb.at(0, 0, 0)), Fb, with_visc, A, rho);
+}
+
 // a6: a_ab = sum_i (f_i - f_i^eq + S_i/2) H_i,ab (Eq. 7) in closed form (O5'):
 //   sum f H = Pi - cs2 p* I,  sum f^eq H = uu,  sum S H = uA + Au.
 __device__ __forceinline__ void hermite_coeff(const Moments& M, const double (&u)[3], const double (&A)[3],
@@ -147,6 +155,26 @@ __device__ __forceinline__ void hermite_coeff(const Moments& M, const double (&u
   a[3] = M.Pi[3] - u[0] * u[1] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
   a[4] = M.Pi[4] - u[0] * u[2] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
   a[5] = M.Pi[5] - u[1] * u[2] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
+}
+
+// a6-a7: Hermite coefficient (Eq. 7), regularized reconstruction (Eq. 6) as one second-order Hermite-space
+// population (see hermite2_populations), aligned store of f*_i(x) into the other buffer.
+template <typename ST>
+__device__ __forceinline__ void collide_store(const KP& P, const Moments& M, const double (&u)[3], const double (&A)[3],
+                                              double (&f)[Q], ST* __restrict__ fout, unsigned k) {
+  double a[6];
+  hermite_coeff(M, u, A, a);
+  const double U[3] = {u[0] + 0.5 * A[0], u[1] + 0.5 * A[1], u[2] + 0.5 * A[2]};
+  double T[6];
+  T[0] = u[0] * u[0] + P.one_m_omega * a[0] + u[0] * A[0];
+  T[1] = u[1] * u[1] + P.one_m_omega * a[1] + u[1] * A[1];
+  T[2] = u[2] * u[2] + P.one_m_omega * a[2] + u[2] * A[2];
+  T[3] = u[0] * u[1] + P.one_m_omega * a[3] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
+  T[4] = u[0] * u[2] + P.one_m_omega * a[4] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
+  T[5] = u[1] * u[2] + P.one_m_omega * a[5] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
+  hermite2_populations(M.p, U, T, f);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) Pop<ST>::store(fout + (size_t)i * P.G.n + k, i, f[i]);
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
@@ -193,20 +221,7 @@ __global__ void __launch_bounds__(128) k_lb(KP P, const ST* __restrict__ fin, ST
     uout[P.G.n + k] = u[1];
     uout[2u * P.G.n + k] = u[2];
   }
-  double a[6];
-  hermite_coeff(M, u, A, a);
-  // a7: Eq. 6 as one second-order Hermite-space population (see hermite2_populations)
-  const double U[3] = {u[0] + 0.5 * A[0], u[1] + 0.5 * A[1], u[2] + 0.5 * A[2]};
-  double T[6];
-  T[0] = u[0] * u[0] + P.one_m_omega * a[0] + u[0] * A[0];
-  T[1] = u[1] * u[1] + P.one_m_omega * a[1] + u[1] * A[1];
-  T[2] = u[2] * u[2] + P.one_m_omega * a[2] + u[2] * A[2];
-  T[3] = u[0] * u[1] + P.one_m_omega * a[3] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
-  T[4] = u[0] * u[2] + P.one_m_omega * a[4] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
-  T[5] = u[1] * u[2] + P.one_m_omega * a[5] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
-  hermite2_populations(M.p, U, T, f);
-#pragma unroll
-  for (int i = 0; i < Q; ++i) Pop<ST>::store(fout + (size_t)i * P.G.n + k, i, f[i]);
+  collide_store<ST>(P, M, u, A, f, fout, k);
 }
 
 // a8: conservative Allen-Cahn update (Eq. 3), forward Euler (R13):
@@ -394,6 +409,8 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
 
 }  // namespace acclb
 
+#include "twophase.cuh"
+
 // ================================================================================================== host / ABI
 using namespace acclb;
 
@@ -407,6 +424,7 @@ struct accLB_ctx {
   void* f[2];
   double* phi[2];
   double* u;
+  double* r;    // D lap phi - kappa div q of the current step (k_lb_tp -> k_advect)
   double* nrm;
   double* tabs;
   double* acc;
@@ -467,7 +485,7 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
 }
 
 struct Carve {
-  size_t f, phi, u, nrm, tabs, acc, stage, total;
+  size_t f, phi, u, r, nrm, tabs, acc, stage, total;
 };
 static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   const size_t n = (size_t)nx * ny * nz;
@@ -475,11 +493,12 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   c.f = align256(27 * n * (p->store_fp32 ? 4 : 8));
   c.phi = p->two_phase ? align256(n * 8) : 0;
   c.u = p->two_phase ? align256(3 * n * 8) : 0;
+  c.r = p->two_phase ? align256(n * 8) : 0;
   c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
   c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
   c.acc = align256(16 * 8);
   c.stage = p->host_staging ? align256(5 * n * 8) : 0;
-  c.total = 2 * c.f + 2 * c.phi + c.u + c.nrm + c.tabs + c.acc + c.stage;
+  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.stage;
   return c;
 }
 
@@ -490,6 +509,47 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   } while (0)
 
 static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+// Tile shapes of the two-phase kernels.
+constexpr int LBT_TX = 32, LBT_TY = 8, LBT_MINB = 2;
+constexpr int ADV_TX = 32, ADV_TY = 8;
+
+// Planes per block along z: enough blocks to load every SM a few times over, chunks of equal length, and no
+// chunk so short that its prologue (4 phi planes, 2 derived planes) dominates.
+static int planes_per_block(int nx, int ny, int nz, int tx, int ty) {
+  const long long tiles = (long long)((nx + tx - 1) / tx) * ((ny + ty - 1) / ty);
+  long long lz = (long long)nz * tiles / (148LL * 12LL);
+  if (lz < 8) lz = 8;
+  if (lz > 64) lz = 64;
+  if (lz > nz) lz = nz;
+  const int chunks = (int)((nz + lz - 1) / lz);
+  return (nz + chunks - 1) / chunks;
+}
+
+template <typename ST>
+static int launch_lb_tp(accLB_ctx* s, int c, int d) {
+  using T = GeoTile<LBT_TX, LBT_TY>;
+  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB>;
+  static thread_local int configured_device = -1;
+  if (configured_device != s->prm.device) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
+    configured_device = s->prm.device;
+  }
+  const int lz = planes_per_block(s->nx, s->ny, s->nz, LBT_TX, LBT_TY);
+  const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
+  LaunchScope ls(s, KIND_LB);
+  kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], s->u, s->r,
+                                                        s->tabs, lz);
+  return ACCLB_OK;
+}
+
+static int launch_advect(accLB_ctx* s, int c, int d) {
+  const int lz = planes_per_block(s->nx, s->ny, s->nz, ADV_TX, ADV_TY);
+  const dim3 grid((s->nx + ADV_TX - 1) / ADV_TX, (s->ny + ADV_TY - 1) / ADV_TY, (s->nz + lz - 1) / lz);
+  LaunchScope ls(s, KIND_AC);
+  k_advect<ADV_TX, ADV_TY><<<grid, ADV_TX * ADV_TY, 0, s->stream>>>(s->kp, s->phi[c], s->u, s->r, s->phi[d], lz);
+  return ACCLB_OK;
+}
 
 extern "C" {
 
@@ -527,6 +587,7 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   s->phi[0] = p->two_phase ? (double*)w : nullptr; w += c.phi;
   s->phi[1] = p->two_phase ? (double*)w : nullptr; w += c.phi;
   s->u = p->two_phase ? (double*)w : nullptr; w += c.u;
+  s->r = p->two_phase ? (double*)w : nullptr; w += c.r;
   s->nrm = p->two_phase ? (double*)w : nullptr; w += c.nrm;
   s->tabs = (double*)w; w += c.tabs;
   s->acc = (double*)w; w += c.acc;
@@ -613,7 +674,14 @@ int accLB_step(accLB_ctx* s, int nsteps) {
   const unsigned nb = blocks_for(s->n, 128);
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
-    if (s->prm.two_phase) {
+    if (s->prm.two_phase && s->variant == 0) {
+      // tiled path: fused LB + geometry (k_lb_tp), then the advective phi update (k_advect)
+      int r = s->prm.store_fp32 ? launch_lb_tp<float>(s, c, d) : launch_lb_tp<double>(s, c, d);
+      if (r) return r;
+      r = launch_advect(s, c, d);
+      if (r) return r;
+    } else if (s->prm.two_phase) {
+      // variant 1: one node per thread, stencils straight from global memory (k_normal, k_lb, k_allen_cahn)
       int r = launch_normal(s);
       if (r) return r;
       {

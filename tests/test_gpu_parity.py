@@ -268,11 +268,38 @@ def test_launch_count_and_errors(acclb):
     sim2 = gpu_sim(acclb, cfg2)
     c0 = sim2.launch_count
     sim2.step(4)
-    assert sim2.launch_count - c0 == 12        # normal + LB + Allen-Cahn per two-phase step
+    assert sim2.launch_count - c0 == 8         # fused LB + advection per two-phase step (tiled path)
+    sim2.set_variant(1)
+    c0 = sim2.launch_count
+    sim2.step(4)
+    assert sim2.launch_count - c0 == 12        # variant 1: normal + LB + Allen-Cahn
     with pytest.raises(acclb.AccLBError):
         sim.step(-1)
     with pytest.raises(acclb.AccLBError):
         acclb.AccLB(31, 32, 32, tau=0.8)
+
+
+@pytest.mark.parametrize("ratio", [1.0, 10.0])
+def test_variant1_flat_kernels_match_oracle_and_default(acclb, ratio):
+    """Variant 1 (one node per thread, stencils from global memory) and the default tiled path agree with the oracle
+    and with each other to rounding; switching variants in mid-run is allowed."""
+    cfg = wl.make_config("droplet", n=40, density_ratio=ratio)
+    a, b, o = gpu_sim(acclb, cfg), gpu_sim(acclb, cfg), cpu_sim(cfg)
+    b.set_variant(1)
+    a.step(30)
+    b.step(30)
+    o.step(30)
+    assert_parity(a, o)
+    assert_parity(b, o)
+    b.set_variant(0)
+    a.step(5)
+    b.step(5)
+    o.step(5)
+    assert_parity(b, o)
+    for x, y in zip(a.moments(), b.moments()):
+        assert (x - y).abs().max().item() <= 1e-12
+    with pytest.raises(acclb.AccLBError):
+        a.set_variant(7)
 
 
 def test_non_default_stream(acclb):
