@@ -34,16 +34,24 @@ __device__ __forceinline__ double lattice_laplacian(V val) {
   return 6.0 * (acc * (1.0 / 216.0) - val(0, 0, 0));
 }
 
+// Shared-memory working set of k_lb_tp for one TX x TY column marching along z.
+//   The D3Q27 stencil weights factorise, w_i = W(cx) W(cy) W(cz) / 216 with W = (1,4,1), so every lattice stencil of
+//   PAPER.md:L104 is evaluated separably: a z combination per (x,y) column first (Sz = (1,4,1), Dz = (+1,0,-1)), then a
+//   3 x 3 stencil in the plane.  Same numbers as the 27-term sums up to rounding order.
 template <int TX, int TY>
 struct GeoTile {
-  static constexpr int PX = TX + 4, PY = TY + 4;  // phi plane with halo 2
-  static constexpr int NX = TX + 2, NY = TY + 2;  // derived-field plane with halo 1
-  static constexpr int NF = 7;                    // n_x n_y n_z q_x q_y q_z |grad phi|
-  double phi[5][PY][PX];                          // ring over z: plane zz lives in slot (zz - z0 + 2) % 5
-  double fld[3][NF][NY][NX];                      // ring over z: plane zz lives in slot (zz - z0 + 1) % 3
+  static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
+  static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
+  double raw[3][PY][PX];     // ring of raw phi planes zc-1, zc, zc+1
+  double Tz[PY][PX];         // Sz phi at plane zc
+  double Dz[PY][PX];         // Dz phi at plane zc
+  double nq[2][6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc (slot zc & 1), q = phi (1 - phi) n
+  double own[2][5][TY][TX];  // g_x g_y g_z |g| lap(phi) of plane zc at the tile's own nodes (slot zc & 1)
 };
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
+// Iteration zc: stage phi(zc+1) -> Sz, Dz of plane zc | derive n, q, g, |g|, lap on plane zc | plane sums of plane zc,
+// then the node update of plane z = zc - 1, whose z combinations need planes zc-2 .. zc (carried in registers).
 template <typename ST, int TX, int TY, int MINB>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
@@ -52,6 +60,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T& S = *reinterpret_cast<T*>(smem_raw);
   constexpr int NT = TX * TY;
+  constexpr int RIM2 = T::PX * T::PY - NT;  // staging items besides the thread's own node
+  constexpr int RIM1 = T::NX * T::NY - NT;  // derive items besides the thread's own node
+  static_assert(RIM2 <= NT && RIM1 <= NT, "at most one rim item per thread");
   const Grid& G = P.G;
   const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * lz;
@@ -60,115 +71,174 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const bool active = x < G.nx && y < G.ny;
   const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
 
-  // phi tile elements this thread stages per plane: element e = tid + l NT of the PY x PX tile
-  constexpr int NPHI = T::PX * T::PY, LP = (NPHI + NT - 1) / NT;
-  unsigned poff[LP];
-#pragma unroll
-  for (int l = 0; l < LP; ++l) {
-    const int e = tid + l * NT;
-    const int j = e / T::PX, i = e % T::PX;
-    poff[l] = (unsigned)pmod(y0 - 2 + j, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 2 + i, G.nx);
+  // rim item of the staging pass: the tid-th element of the PY x PX plane that is not an own node
+  int r2 = -1;  // linear index j * PX + i in a phi plane
+  unsigned r2off = 0;
+  if (tid < RIM2) {
+    int j, i;
+    if (tid < 2 * T::PX) { j = tid / T::PX; i = tid % T::PX; }                                   // rows 0, 1
+    else if (tid < 4 * T::PX) { j = TY + tid / T::PX; i = tid % T::PX; }                         // rows PY-2, PY-1
+    else { const int e = tid - 4 * T::PX; j = 2 + e / 4; i = (e & 3) < 2 ? (e & 3) : TX + (e & 3); }  // columns
+    r2 = j * T::PX + i;
+    r2off = (unsigned)pmod(y0 - 2 + j, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 2 + i, G.nx);
   }
-  auto stage_phi = [&](int zz) {  // plane zz (unwrapped) -> ring slot
-    const double* src = phi + (size_t)pmod(zz, G.nz) * plane;
-    double* dst = &S.phi[(zz - z0 + 2) % 5][0][0];
-#pragma unroll
-    for (int l = 0; l < LP; ++l) {
-      const int e = tid + l * NT;
-      if (e < NPHI) dst[e] = __ldg(src + poff[l]);
-    }
-  };
-  // n = g / (|g| + 1e-12) (R17), q = phi (1 - phi) n (Eq. 3), |g|, on the tile + 1 rim of plane zz
-  auto derive = [&](int zz) {
-    const int sp = (zz - z0 + 2) % 5, sm = (zz - z0 + 1) % 5, sq = (zz - z0 + 3) % 5;
-    const int so = (zz - z0 + 1) % 3;
-    constexpr int NN = T::NX * T::NY;
-    for (int e = tid; e < NN; e += NT) {
-      const int j = e / T::NX, i = e % T::NX;
-      auto val = [&](int dz, int dy, int dx) {
-        return S.phi[dz < 0 ? sm : (dz > 0 ? sq : sp)][j + 1 + dy][i + 1 + dx];
-      };
-      const double gx = lattice_derivative<0>(val), gy = lattice_derivative<1>(val), gz = lattice_derivative<2>(val);
-      const double gn = sqrt(gx * gx + gy * gy + gz * gz);
-      const double inv = 1.0 / (gn + 1e-12);
-      const double ph = val(0, 0, 0), pq = ph * (1.0 - ph);
-      const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
-      S.fld[so][0][j][i] = nx_;
-      S.fld[so][1][j][i] = ny_;
-      S.fld[so][2][j][i] = nz_;
-      S.fld[so][3][j][i] = pq * nx_;
-      S.fld[so][4][j][i] = pq * ny_;
-      S.fld[so][5][j][i] = pq * nz_;
-      S.fld[so][6][j][i] = gn;
-    }
-  };
+  const int o2 = (ty + 2) * T::PX + (tx + 2);
+  const unsigned o2off = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
+  // rim item of the derive pass: element (j, i) of the NY x NX plane that is not an own node
+  int r1j = -1, r1i = 0;
+  if (tid < RIM1) {
+    if (tid < T::NX) { r1j = 0; r1i = tid; }
+    else if (tid < 2 * T::NX) { r1j = T::NY - 1; r1i = tid - T::NX; }
+    else { const int e = tid - 2 * T::NX; r1j = 1 + (e >> 1); r1i = (e & 1) ? T::NX - 1 : 0; }
+  }
 
-  // prologue: phi planes z0-2 .. z0+1, derived planes z0-1, z0
-  stage_phi(z0 - 2);
-  stage_phi(z0 - 1);
-  stage_phi(z0);
-  stage_phi(z0 + 1);
+  const int xw = pmod(x, G.nx), yw = pmod(y, G.ny);
+  const int xs[3] = {wrap_dec(xw, G.nx), xw, wrap_inc(xw, G.nx)};
+  const unsigned yrow[3] = {(unsigned)wrap_dec(yw, G.ny) * (unsigned)G.nx, (unsigned)yw * (unsigned)G.nx,
+                            (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx};
+
+  // stage raw phi planes z0-2 and z0-1
+  {
+    const double* s0 = phi + (size_t)pmod(z0 - 2, G.nz) * plane;
+    const double* s1 = phi + (size_t)pmod(z0 - 1, G.nz) * plane;
+    double* d0 = &S.raw[0][0][0];
+    double* d1 = &S.raw[1][0][0];
+    d0[o2] = __ldg(s0 + o2off);
+    d1[o2] = __ldg(s1 + o2off);
+    if (r2 >= 0) {
+      d0[r2] = __ldg(s0 + r2off);
+      d1[r2] = __ldg(s1 + r2off);
+    }
+  }
+  double an0 = 0.0, an1 = 0.0, bn0 = 0.0, bn1 = 0.0;  // plane sums of n at planes zc-2, zc-1
+  double aq0 = 0.0, aq1 = 0.0, bq0 = 0.0, bq1 = 0.0;  // plane sums of q
   __syncthreads();
-  derive(z0 - 1);
-  derive(z0);
 
-  const int xs[3] = {wrap_dec(x < G.nx ? x : 0, G.nx), x < G.nx ? x : 0, wrap_inc(x < G.nx ? x : 0, G.nx)};
-  const int yy = y < G.ny ? y : 0;
-  const unsigned yrow[3] = {(unsigned)wrap_dec(yy, G.ny) * (unsigned)G.nx, (unsigned)yy * (unsigned)G.nx,
-                            (unsigned)wrap_inc(yy, G.ny) * (unsigned)G.nx};
-
-  for (int z = z0; z < z1; ++z) {
-    stage_phi(z + 2);
-    __syncthreads();
-    derive(z + 1);
-    __syncthreads();
-    if (!active) continue;  // barriers above are executed by every thread: the loop bounds are block-uniform
-
-    const int fm = (z - z0) % 3, f0 = (z - z0 + 1) % 3, fp = (z - z0 + 2) % 3;
-    auto fld = [&](int c, int dz, int dy, int dx) {
-      return S.fld[dz < 0 ? fm : (dz > 0 ? fp : f0)][c][ty + 1 + dy][tx + 1 + dx];
-    };
-    const int pm = (z - z0 + 1) % 5, p0 = (z - z0 + 2) % 5, pp = (z - z0 + 3) % 5;
-    auto ph = [&](int dz, int dy, int dx) { return S.phi[dz < 0 ? pm : (dz > 0 ? pp : p0)][ty + 2 + dy][tx + 2 + dx]; };
-
-    // a3: kappa_c = div n, div q, lap phi by the lattice stencils
-    const double kc = lattice_derivative<0>([&](int dz, int dy, int dx) { return fld(0, dz, dy, dx); }) +
-                      lattice_derivative<1>([&](int dz, int dy, int dx) { return fld(1, dz, dy, dx); }) +
-                      lattice_derivative<2>([&](int dz, int dy, int dx) { return fld(2, dz, dy, dx); });
-    const double divq = lattice_derivative<0>([&](int dz, int dy, int dx) { return fld(3, dz, dy, dx); }) +
-                        lattice_derivative<1>([&](int dz, int dy, int dx) { return fld(4, dz, dy, dx); }) +
-                        lattice_derivative<2>([&](int dz, int dy, int dx) { return fld(5, dz, dy, dx); });
-    const double lap = lattice_laplacian(ph);
-    const double gn = fld(6, 0, 0, 0);
-    const double gs = gn + 1e-12;  // g = n (|g| + 1e-12) up to rounding
-    const double g[3] = {fld(0, 0, 0, 0) * gs, fld(1, 0, 0, 0) * gs, fld(2, 0, 0, 0) * gs};
-    const double phi0 = ph(0, 0, 0);
-
-    const unsigned k = (unsigned)z * plane + yrow[1] + (unsigned)xs[1];
-    rout[k] = P.D * lap - P.kappa * divq;  // phi-only part of Eq. 3
-
-    // a1: pull-stream
-    Nbr nb;
-    nb.x[0] = xs[0]; nb.x[1] = xs[1]; nb.x[2] = xs[2];
+  for (int zc = z0 - 1; zc <= z1; ++zc) {
+    const int it = zc - (z0 - 1);  // 0, 1, 2, ...
+    // ---- stage phi(zc+1); z combinations of plane zc
     {
-      const unsigned zr[3] = {(unsigned)wrap_dec(z, G.nz) * plane, (unsigned)z * plane, (unsigned)wrap_inc(z, G.nz) * plane};
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) nb.row[a][b] = zr[a] + yrow[b];
+      const double* src = phi + (size_t)pmod(zc + 1, G.nz) * plane;
+      const double* rm = &S.raw[it % 3][0][0];        // plane zc-1
+      const double* rc = &S.raw[(it + 1) % 3][0][0];  // plane zc
+      double* rp = &S.raw[(it + 2) % 3][0][0];        // plane zc+1
+      double* tz = &S.Tz[0][0];
+      double* dz = &S.Dz[0][0];
+      const double v = __ldg(src + o2off);
+      const double m = rm[o2];
+      rp[o2] = v;
+      tz[o2] = fma(4.0, rc[o2], m + v);
+      dz[o2] = v - m;
+      if (r2 >= 0) {
+        const double v2 = __ldg(src + r2off);
+        const double m2 = rm[r2];
+        rp[r2] = v2;
+        tz[r2] = fma(4.0, rc[r2], m2 + v2);
+        dz[r2] = v2 - m2;
+      }
     }
-    double f[Q];
-    pull27<ST>(fin, G, nb, f);
-    Moments M;
-    moments_of(f, M);
-    double Fb[3], A[3], rho;
-    body_force(P, tabs, x, y, z, Fb);
-    accel_from_geometry(P, M, g, gn, kc, phi0, Fb, true, A, rho);
-    const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
-    uout[k] = u[0];
-    uout[G.n + k] = u[1];
-    uout[2u * G.n + k] = u[2];
-    collide_store<ST>(P, M, u, A, f, fout, k);
+    __syncthreads();
+    // ---- derive n, q (tile + 1 rim) and g, |g|, lap (own nodes) on plane zc           PAPER.md:L61, L104; R17
+    {
+      const int slot = zc & 1;
+      const double* rc = &S.raw[(it + 1) % 3][0][0];
+      auto derive = [&](int j, int i, bool own_node) {  // (j, i) in the NY x NX plane; centre (j+1, i+1) in a phi plane
+        const double* t = &S.Tz[j][i];
+        const double* d = &S.Dz[j][i];
+        constexpr int PX = T::PX;
+        const double t00 = t[0], t01 = t[1], t02 = t[2], t10 = t[PX], t11 = t[PX + 1], t12 = t[PX + 2];
+        const double t20 = t[2 * PX], t21 = t[2 * PX + 1], t22 = t[2 * PX + 2];
+        const double gx = (1.0 / 72.0) * fma(4.0, t12 - t10, (t02 - t00) + (t22 - t20));
+        const double gy = (1.0 / 72.0) * fma(4.0, t21 - t01, (t20 - t00) + (t22 - t02));
+        const double r0 = fma(4.0, d[1], d[0] + d[2]);
+        const double r1 = fma(4.0, d[PX + 1], d[PX] + d[PX + 2]);
+        const double r2_ = fma(4.0, d[2 * PX + 1], d[2 * PX] + d[2 * PX + 2]);
+        const double gz = (1.0 / 72.0) * fma(4.0, r1, r0 + r2_);
+        const double gn = sqrt(fma(gx, gx, fma(gy, gy, gz * gz)));
+        const double inv = 1.0 / (gn + 1e-12);
+        const double ph = rc[(j + 1) * PX + (i + 1)];
+        const double pq = ph * (1.0 - ph);
+        const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
+        S.nq[slot][0][j][i] = nx_;
+        S.nq[slot][1][j][i] = ny_;
+        S.nq[slot][2][j][i] = nz_;
+        S.nq[slot][3][j][i] = pq * nx_;
+        S.nq[slot][4][j][i] = pq * ny_;
+        S.nq[slot][5][j][i] = pq * nz_;
+        if (own_node) {
+          const double s0 = fma(4.0, t01, t00 + t02), s1 = fma(4.0, t11, t10 + t12), s2 = fma(4.0, t21, t20 + t22);
+          const double lap = 6.0 * (fma(4.0, s1, s0 + s2) * (1.0 / 216.0) - ph);  // R7
+          S.own[slot][0][j - 1][i - 1] = gx;
+          S.own[slot][1][j - 1][i - 1] = gy;
+          S.own[slot][2][j - 1][i - 1] = gz;
+          S.own[slot][3][j - 1][i - 1] = gn;
+          S.own[slot][4][j - 1][i - 1] = lap;
+        }
+      };
+      derive(ty + 1, tx + 1, true);
+      if (r1j >= 0) derive(r1j, r1i, false);
+    }
+    __syncthreads();
+    // ---- plane sums of plane zc at the own node:  a = Dx Sy v_x + Sx Dy v_y,  b = Sx Sy v_z
+    double an2, bn2, aq2, bq2;
+    {
+      const int slot = zc & 1;
+      constexpr int NX = T::NX;
+      auto plane_sums = [&](int c0, double& a, double& b) {
+        const double* vx = &S.nq[slot][c0][ty][tx];
+        const double* vy = &S.nq[slot][c0 + 1][ty][tx];
+        const double* vz = &S.nq[slot][c0 + 2][ty][tx];
+        const double ax = fma(4.0, vx[NX + 2] - vx[NX], (vx[2] - vx[0]) + (vx[2 * NX + 2] - vx[2 * NX]));
+        const double ay = fma(4.0, vy[2 * NX + 1] - vy[1], (vy[2 * NX] - vy[0]) + (vy[2 * NX + 2] - vy[2]));
+        a = ax + ay;
+        const double r0 = fma(4.0, vz[1], vz[0] + vz[2]);
+        const double r1 = fma(4.0, vz[NX + 1], vz[NX] + vz[NX + 2]);
+        const double r2_ = fma(4.0, vz[2 * NX + 1], vz[2 * NX] + vz[2 * NX + 2]);
+        b = fma(4.0, r1, r0 + r2_);
+      };
+      plane_sums(0, an2, bn2);
+      plane_sums(3, aq2, bq2);
+    }
+    const int z = zc - 1;
+    if (z >= z0 && active) {
+      // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
+      const double kc = (1.0 / 72.0) * (fma(4.0, an1, an0 + an2) + (bn2 - bn0));
+      const double divq = (1.0 / 72.0) * (fma(4.0, aq1, aq0 + aq2) + (bq2 - bq0));
+      const int so = z & 1;
+      const double g[3] = {S.own[so][0][ty][tx], S.own[so][1][ty][tx], S.own[so][2][ty][tx]};
+      const double gn = S.own[so][3][ty][tx];
+      const double lap = S.own[so][4][ty][tx];
+      const double phi0 = S.raw[it % 3][ty + 2][tx + 2];  // plane zc-1 = z
+
+      const unsigned k = (unsigned)z * plane + yrow[1] + (unsigned)xs[1];
+      rout[k] = P.D * lap - P.kappa * divq;  // phi-only part of Eq. 3
+
+      // a1: pull-stream
+      Nbr nb;
+      nb.x[0] = xs[0]; nb.x[1] = xs[1]; nb.x[2] = xs[2];
+      {
+        const unsigned zr[3] = {(unsigned)wrap_dec(z, G.nz) * plane, (unsigned)z * plane,
+                                (unsigned)wrap_inc(z, G.nz) * plane};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int b = 0; b < 3; ++b) nb.row[a][b] = zr[a] + yrow[b];
+      }
+      double f[Q];
+      pull27<ST>(fin, G, nb, f);
+      Moments M;
+      moments_of(f, M);
+      double Fb[3], A[3], rho;
+      body_force(P, tabs, x, y, z, Fb);
+      accel_from_geometry(P, M, g, gn, kc, phi0, Fb, true, A, rho);
+      const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
+      uout[k] = u[0];
+      uout[G.n + k] = u[1];
+      uout[2u * G.n + k] = u[2];
+      collide_store<ST>(P, M, u, A, f, fout, k);
+    }
+    an0 = an1; an1 = an2; bn0 = bn1; bn1 = bn2;
+    aq0 = aq1; aq1 = aq2; bq0 = bq1; bq1 = bq2;
   }
 }
 
