@@ -270,24 +270,29 @@ def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=T
 
 
 def roofline_of(meas, steps, fp32):
-    """Roofline object for the dominant kernel (the fused LB step k_lb), from its CUDA-event durations."""
+    """Roofline object for the dominant kernel, from its CUDA-event durations inside the timed region.  The dominant
+    kernel is k_step_tp (the whole two-phase step as one persistent kernel: algorithmic bytes = 54 populations + phi
+    read + phi written per node) or k_lb (the fused LB step: 54 populations per node)."""
     n3 = meas["n"] ** 3
-    ms_lb, cnt_lb = meas["kernels"]["k_lb"]
+    kernels = {k: v for k, v in meas["kernels"].items() if v[1]}
+    name = max(kernels, key=lambda k: kernels[k][0])
+    ms_k, cnt_k = kernels[name]
+    bpl = step_bytes_per_lup(fp32, meas["two_phase"]) if name == "k_step_tp" else lb_bytes_per_lup(fp32)
     peak, how = hbm_peak()
-    per_launch_ms = ms_lb / max(cnt_lb, 1)
-    achieved = lb_bytes_per_lup(fp32) * n3 / (per_launch_ms * 1e-3) / 1e9
-    total_ms = sum(v[0] for v in meas["kernels"].values())
-    r = {"bound": "hbm", "kernel": "k_lb", "achieved": achieved, "peak": peak, "peak_source": how, "unit": "GB/s",
-         "frac": achieved / peak, "traffic": None, "bytes_per_launch": lb_bytes_per_lup(fp32) * n3,
-         "kernel_ms_per_launch": per_launch_ms, "kernel_share_of_step": ms_lb / total_ms if total_ms else None,
-         "kernels_ms_per_step": {k: v[0] / steps for k, v in meas["kernels"].items() if v[1]},
+    per_launch_ms = ms_k / max(cnt_k, 1)
+    achieved = bpl * n3 / (per_launch_ms * 1e-3) / 1e9
+    total_ms = sum(v[0] for v in kernels.values())
+    r = {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": peak, "peak_source": how, "unit": "GB/s",
+         "frac": achieved / peak, "traffic": None, "bytes_per_launch": bpl * n3, "bytes_per_lup": bpl,
+         "kernel_ms_per_launch": per_launch_ms, "kernel_share_of_step": ms_k / total_ms if total_ms else None,
+         "kernels_ms_per_step": {k: v[0] / steps for k, v in kernels.items()},
          "step_bytes_per_lup": step_bytes_per_lup(fp32, meas["two_phase"])}
     r["step_achieved"] = r["step_bytes_per_lup"] * n3 * steps / (meas["ms"] * 1e-3) / 1e9
     r["step_frac"] = r["step_achieved"] / peak
-    t = ROOT / "profiles" / "traffic.json"  # dram bytes per launch of k_lb from the committed ncu --set full capture
+    t = ROOT / "profiles" / "traffic.json"  # dram bytes per launch of the kernel from the committed ncu --set full capture
     try:
         tj = json.loads(t.read_text())
-        key = f"{'two' if meas['two_phase'] else 'single'}_{'fp32' if fp32 else 'fp64'}_{meas['n']}"
+        key = f"{name}_{'two' if meas['two_phase'] else 'single'}_{'fp32' if fp32 else 'fp64'}_{meas['n']}"
         r["traffic"] = tj.get(key)
     except Exception:
         pass

@@ -104,8 +104,9 @@ long long accLB_launch_count(const accLB_ctx* ctx);
  * the context's stream; accLB_profile_read synchronises the stream, adds the elapsed milliseconds and launch
  * counts per kernel kind into ms[k], count[k] for k < min(n, ACCLB_NKERNELS) (HOST pointers) and clears the
  * record.  Kinds: 0 k_normal, 1 k_lb (the fused LB step), 2 k_allen_cahn, 3 k_init, 4 k_moments,
- * 5 k_diagnostics.  This is how bench.py measures the dominant kernel's duration inside the timed region. */
-#define ACCLB_NKERNELS 6
+ * 5 k_diagnostics, 6 k_step_tp (the whole two-phase step as one persistent kernel).  This is how bench.py measures
+ * the dominant kernel's duration inside the timed region. */
+#define ACCLB_NKERNELS 7
 int accLB_profile(accLB_ctx* ctx, int enable);
 int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
 

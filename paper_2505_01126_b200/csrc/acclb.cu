@@ -95,11 +95,10 @@ __device__ __forceinline__ void pull27(const ST* __restrict__ fin, const Grid& G
 //   F^s = -gamma (3 delta/2) kappa_c |g| g (L102, R8);  F^p = -p* cs2 grad rho (L102);
 //   F^nu = -((tau-1/2)/tau) (Pi - p* cs2 I - ut ut) . grad rho (L104, R9), ut = m + (F^s+F^p+F^b)/(2 rho);
 //   F = F^s + F^p + F^nu + F^b (Eq. 8).
-__device__ __forceinline__ void accel_from_geometry(const KP& P, const Moments& M, const double (&g)[3], double gn,
-                                                    double kc, double phi0, const double (&Fb)[3], bool with_visc,
-                                                    double (&A)[3], double& rho) {
+//   fs = -gamma (3 delta/2) kappa_c |g| is passed in (F^s = fs g).
+__device__ __forceinline__ void accel_from_gc(const KP& P, const Moments& M, const double (&g)[3], double fs, double phi0,
+                                              const double (&Fb)[3], bool with_visc, double (&A)[3], double& rho) {
   rho = P.rho_g + P.drho * phi0;
-  const double fs = -P.sig15w * kc * gn;
   const double fp = -M.p * (1.0 / 3.0) * P.drho;
   double F[3];
 #pragma unroll
@@ -117,6 +116,12 @@ __device__ __forceinline__ void accel_from_geometry(const KP& P, const Moments& 
   }
   const double ir = 1.0 / rho;
   A[0] = F[0] * ir; A[1] = F[1] * ir; A[2] = F[2] * ir;
+}
+
+__device__ __forceinline__ void accel_from_geometry(const KP& P, const Moments& M, const double (&g)[3], double gn,
+                                                    double kc, double phi0, const double (&Fb)[3], bool with_visc,
+                                                    double (&A)[3], double& rho) {
+  accel_from_gc(P, M, g, -P.sig15w * kc * gn, phi0, Fb, with_visc, A, rho);
 }
 
 // a3-a5 for the one-node-per-thread kernels: g = grad phi and kappa_c = div n by the lattice stencils
@@ -410,6 +415,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
 }  // namespace acclb
 
 #include "twophase.cuh"
+#include "pipeline.cuh"
 
 // ================================================================================================== host / ABI
 using namespace acclb;
@@ -428,6 +434,9 @@ struct accLB_ctx {
   double* nrm;
   double* tabs;
   double* acc;
+  double* rings;  // pipeline ring buffers: n(3) | g,c(4) | r | u(3) | fz, PIPE_RING planes each (two-phase)
+  int* sync;      // pipeline counters: ticket | done[4][nz + 4]
+  int pipe_grid;  // resident blocks of k_step_tp
   double* stage;  // [5 n] rho | u(3) | phi, host_staging only
   int cur;        // f[cur], phi[cur] hold the current state
   long long step;
@@ -458,7 +467,7 @@ struct LaunchScope {
     }
   }
 };
-enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5 };
+enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_STEP = 6 };
 
 static thread_local char g_err[512] = "";
 
@@ -485,7 +494,7 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
 }
 
 struct Carve {
-  size_t f, phi, u, r, nrm, tabs, acc, stage, total;
+  size_t f, phi, u, r, nrm, tabs, acc, rings, sync, stage, total;
 };
 static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   const size_t n = (size_t)nx * ny * nz;
@@ -497,8 +506,10 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
   c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
   c.acc = align256(16 * 8);
+  c.rings = p->two_phase ? align256((size_t)12 * PIPE_RING * nx * ny * 8) : 0;
+  c.sync = p->two_phase ? align256((size_t)(1 + 4 * (nz + 4)) * 4) : 0;
   c.stage = p->host_staging ? align256(5 * n * 8) : 0;
-  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.stage;
+  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.rings + c.sync + c.stage;
   return c;
 }
 
@@ -551,6 +562,50 @@ static int launch_advect(accLB_ctx* s, int c, int d) {
   return ACCLB_OK;
 }
 
+// The two-phase step as one persistent pipeline kernel (pipeline.cuh).
+constexpr int PIPE_MINB = 3;
+
+template <typename ST>
+static int launch_step_tp(accLB_ctx* s, int c, int d) {
+  auto kern = k_step_tp<ST, PIPE_MINB>;
+  if (s->pipe_grid == 0) {
+    int per_sm = 0, sms = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PIPE_THREADS, 0));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->prm.device));
+    if (per_sm < 1) return fail(ACCLB_ECUDA, "k_step_tp: no resident block fits an SM");
+    s->pipe_grid = per_sm * sms;
+  }
+  PipeArgs a;
+  a.P = s->kp;
+  a.fin = s->f[c];
+  a.fout = s->f[d];
+  a.phi = s->phi[c];
+  a.phi_new = s->phi[d];
+  a.tabs = s->tabs;
+  const size_t plane = (size_t)s->nx * s->ny;
+  double* w = s->rings;
+  a.ring_n = w; w += 3 * PIPE_RING * plane;
+  a.ring_gc = w; w += 4 * PIPE_RING * plane;
+  a.ring_r = w; w += PIPE_RING * plane;
+  a.ring_u = w; w += 3 * PIPE_RING * plane;
+  a.ring_fz = w;
+  a.ticket = s->sync;
+  a.done = s->sync + 1;
+  a.tiles_x = (s->nx + PIPE_TX - 1) / PIPE_TX;
+  a.tiles_y = (s->ny + PIPE_TY - 1) / PIPE_TY;
+  a.tiles = a.tiles_x * a.tiles_y;
+  a.lb_items = (int)((plane + PIPE_THREADS - 1) / PIPE_THREADS);
+  a.per_macro = 3 * a.tiles + a.lb_items;
+  const long long total = (long long)(s->nz + 5) * a.per_macro;
+  if (total >= 2000000000LL) return fail(ACCLB_EINVAL, "k_step_tp: too many work items");
+  a.total = (int)total;
+  CK(cudaMemsetAsync(s->sync, 0, (size_t)(1 + 4 * (s->nz + 4)) * 4, s->stream));
+  const int grid = (int)(total < s->pipe_grid ? total : s->pipe_grid);
+  LaunchScope ls(s, KIND_STEP);
+  kern<<<grid, PIPE_THREADS, 0, s->stream>>>(a);
+  return ACCLB_OK;
+}
+
 extern "C" {
 
 size_t accLB_workspace_bytes(int nx, int ny, int nz, const accLB_params* p) {
@@ -591,6 +646,9 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   s->nrm = p->two_phase ? (double*)w : nullptr; w += c.nrm;
   s->tabs = (double*)w; w += c.tabs;
   s->acc = (double*)w; w += c.acc;
+  s->rings = p->two_phase ? (double*)w : nullptr; w += c.rings;
+  s->sync = p->two_phase ? (int*)w : nullptr; w += c.sync;
+  s->pipe_grid = 0;
   s->stage = p->host_staging ? (double*)w : nullptr; w += c.stage;
   s->cur = 0; s->step = 0; s->launches = 0; s->variant = 0; s->profiling = 0;
 
@@ -675,7 +733,11 @@ int accLB_step(accLB_ctx* s, int nsteps) {
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
     if (s->prm.two_phase && s->variant == 0) {
-      // tiled path: fused LB + geometry (k_lb_tp), then the advective phi update (k_advect)
+      // default: the whole step as one persistent pipeline kernel (k_step_tp)
+      int r = s->prm.store_fp32 ? launch_step_tp<float>(s, c, d) : launch_step_tp<double>(s, c, d);
+      if (r) return r;
+    } else if (s->prm.two_phase && s->variant == 2) {
+      // variant 2: fused LB + geometry on z-marching tiles (k_lb_tp), then the advective phi update (k_advect)
       int r = s->prm.store_fp32 ? launch_lb_tp<float>(s, c, d) : launch_lb_tp<double>(s, c, d);
       if (r) return r;
       r = launch_advect(s, c, d);
@@ -814,7 +876,7 @@ long long accLB_launch_count(const accLB_ctx* s) { return s ? s->launches : 0; }
 
 int accLB_set_variant(accLB_ctx* s, int variant) {
   if (!s) return fail(ACCLB_EINVAL, "accLB_set_variant: NULL context");
-  if (variant < 0 || variant > 1) return fail(ACCLB_EINVAL, "accLB_set_variant: unknown variant %d", variant);
+  if (variant < 0 || variant > 2) return fail(ACCLB_EINVAL, "accLB_set_variant: unknown variant %d", variant);
   s->variant = variant;
   return ACCLB_OK;
 }
