@@ -42,10 +42,12 @@ struct KP {
 // population storage: fp64, or fp32 deviation from the lattice weight (R22)
 template <typename ST> struct Pop;
 template <> struct Pop<double> {
+  static __device__ __forceinline__ double from_storage(double v, int) { return v; }
   static __device__ __forceinline__ double load(const double* p, int) { return __ldcs(p); }
   static __device__ __forceinline__ void store(double* p, int, double v) { __stcs(p, v); }
 };
 template <> struct Pop<float> {
+  static __device__ __forceinline__ double from_storage(float v, int i) { return (double)v + w_of(i); }
   static __device__ __forceinline__ double load(const float* p, int i) { return (double)__ldcs(p) + w_of(i); }
   static __device__ __forceinline__ void store(float* p, int i, double v) { __stcs(p, (float)(v - w_of(i))); }
 };
@@ -180,6 +182,13 @@ __device__ __forceinline__ void collide_store(const KP& P, const Moments& M, con
   hermite2_populations(M.p, U, T, f);
 #pragma unroll
   for (int i = 0; i < Q; ++i) Pop<ST>::store(fout + (size_t)i * P.G.n + k, i, f[i]);
+}
+
+template <typename ST>
+__device__ __forceinline__ void collide_store(const KP& P, const Moments& M, const double (&u)[3], const double (&A)[3],
+                                              ST* __restrict__ fout, unsigned k) {
+  double f[Q];
+  collide_store<ST>(P, M, u, A, f, fout, k);
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
@@ -434,7 +443,7 @@ struct accLB_ctx {
   double* nrm;
   double* tabs;
   double* acc;
-  double* rings;  // pipeline ring buffers: n(3) | g,c(4) | r | u(3) | fz, PIPE_RING planes each (two-phase)
+  double* rings;  // pipeline ring buffers: n(3) | g,c(4) | r | u(3) | fz, a few planes each (two-phase)
   int* sync;      // pipeline counters: ticket | done[4][nz + 4]
   int pipe_grid;  // resident blocks of k_step_tp
   double* stage;  // [5 n] rho | u(3) | phi, host_staging only
@@ -506,7 +515,7 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
   c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
   c.acc = align256(16 * 8);
-  c.rings = p->two_phase ? align256((size_t)12 * PIPE_RING * nx * ny * 8) : 0;
+  c.rings = p->two_phase ? align256((size_t)PIPE_RING_DOUBLES * nx * ny * 8) : 0;
   c.sync = p->two_phase ? align256((size_t)(1 + 4 * (nz + 4)) * 4) : 0;
   c.stage = p->host_staging ? align256(5 * n * 8) : 0;
   c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.rings + c.sync + c.stage;
@@ -539,7 +548,7 @@ static int planes_per_block(int nx, int ny, int nz, int tx, int ty) {
 
 template <typename ST>
 static int launch_lb_tp(accLB_ctx* s, int c, int d) {
-  using T = GeoTile<LBT_TX, LBT_TY>;
+  using T = GeoTile<ST, LBT_TX, LBT_TY>;
   auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB>;
   static thread_local int configured_device = -1;
   if (configured_device != s->prm.device) {
@@ -584,10 +593,10 @@ static int launch_step_tp(accLB_ctx* s, int c, int d) {
   a.tabs = s->tabs;
   const size_t plane = (size_t)s->nx * s->ny;
   double* w = s->rings;
-  a.ring_n = w; w += 3 * PIPE_RING * plane;
-  a.ring_gc = w; w += 4 * PIPE_RING * plane;
-  a.ring_r = w; w += PIPE_RING * plane;
-  a.ring_u = w; w += 3 * PIPE_RING * plane;
+  a.ring_n = w; w += 3 * RING_N * plane;
+  a.ring_gc = w; w += 4 * RING_GC * plane;
+  a.ring_r = w; w += RING_R * plane;
+  a.ring_u = w; w += 3 * RING_U * plane;
   a.ring_fz = w;
   a.ticket = s->sync;
   a.done = s->sync + 1;
@@ -596,7 +605,7 @@ static int launch_step_tp(accLB_ctx* s, int c, int d) {
   a.tiles = a.tiles_x * a.tiles_y;
   a.lb_items = (int)((plane + PIPE_THREADS - 1) / PIPE_THREADS);
   a.per_macro = 3 * a.tiles + a.lb_items;
-  const long long total = (long long)(s->nz + 5) * a.per_macro;
+  const long long total = (long long)(s->nz + 3 + LAG_ADV) * a.per_macro;
   if (total >= 2000000000LL) return fail(ACCLB_EINVAL, "k_step_tp: too many work items");
   a.total = (int)total;
   CK(cudaMemsetAsync(s->sync, 0, (size_t)(1 + 4 * (s->nz + 4)) * 4, s->stream));
@@ -733,14 +742,14 @@ int accLB_step(accLB_ctx* s, int nsteps) {
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
     if (s->prm.two_phase && s->variant == 0) {
-      // default: the whole step as one persistent pipeline kernel (k_step_tp)
-      int r = s->prm.store_fp32 ? launch_step_tp<float>(s, c, d) : launch_step_tp<double>(s, c, d);
-      if (r) return r;
-    } else if (s->prm.two_phase && s->variant == 2) {
-      // variant 2: fused LB + geometry on z-marching tiles (k_lb_tp), then the advective phi update (k_advect)
+      // default: fused LB + geometry on z-marching tiles (k_lb_tp), then the advective phi update (k_advect)
       int r = s->prm.store_fp32 ? launch_lb_tp<float>(s, c, d) : launch_lb_tp<double>(s, c, d);
       if (r) return r;
       r = launch_advect(s, c, d);
+      if (r) return r;
+    } else if (s->prm.two_phase && s->variant == 2) {
+      // variant 2: the whole step as one persistent pipeline kernel (k_step_tp, pipeline.cuh)
+      int r = s->prm.store_fp32 ? launch_step_tp<float>(s, c, d) : launch_step_tp<double>(s, c, d);
       if (r) return r;
     } else if (s->prm.two_phase) {
       // variant 1: one node per thread, stencils straight from global memory (k_normal, k_lb, k_allen_cahn)

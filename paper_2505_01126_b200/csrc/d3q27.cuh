@@ -29,15 +29,17 @@ struct Moments {
   double p, m[3], Pi[6];
 };
 
-__device__ __forceinline__ void moments_of(const double (&f)[Q], Moments& M) {
-  double p = f[13];
+template <class F>
+__device__ __forceinline__ void moments_of(F f_of, Moments& M) {  // f_of(i) = f_i, each i asked for once
+  double p = f_of(13);
   double mx = 0.0, my = 0.0, mz = 0.0;
   double pxx = 0.0, pyy = 0.0, pzz = 0.0, pxy = 0.0, pxz = 0.0, pyz = 0.0;
 #pragma unroll
   for (int i = 0; i < 13; ++i) {
     const int cx = cx_of(i), cy = cy_of(i), cz = cz_of(i);
-    const double s = f[i] + f[26 - i];
-    const double d = f[i] - f[26 - i];
+    const double fa = f_of(i), fb = f_of(26 - i);
+    const double s = fa + fb;
+    const double d = fa - fb;
     p += s;
     if (cx == 1) mx += d;
     if (cx == -1) mx -= d;
@@ -58,6 +60,10 @@ __device__ __forceinline__ void moments_of(const double (&f)[Q], Moments& M) {
   M.p = p;
   M.m[0] = mx; M.m[1] = my; M.m[2] = mz;
   M.Pi[0] = pxx; M.Pi[1] = pyy; M.Pi[2] = pzz; M.Pi[3] = pxy; M.Pi[4] = pxz; M.Pi[5] = pyz;
+}
+
+__device__ __forceinline__ void moments_of(const double (&f)[Q], Moments& M) {
+  moments_of([&](int i) { return f[i]; }, M);
 }
 
 // Second-order Hermite-space population

@@ -16,7 +16,7 @@
 // little else.  The fp64-ALU-bound stages (N, K, ADV) share the SMs with the HBM-bound LB items and hide under them.
 //
 // Scheduling.  Blocks take tickets from one global counter; ticket -> (macro step m, stage, item).  Macro step m holds,
-// in this order, N(zz = m-2), LB(zz = m-4), K(zz = m-3), ADV(zz = m-5).  zz is the unwrapped plane coordinate,
+// in this order, N(zz = m-2), LB(zz = m-4), K(zz = m-3), ADV(zz = m-6).  zz is the unwrapped plane coordinate,
 // z = zz mod nz; N covers zz in [-2, nz+1], K and LB [-1, nz], ADV [0, nz-1]: the two wrap-around planes are simply
 // processed twice (LB is idempotent: it reads buffer A and writes buffer B), so the pipeline is linear and the
 // periodic wrap needs no special case.  An item waits (one thread spins on an acquire load) until the per-plane
@@ -31,7 +31,12 @@ namespace acclb {
 
 constexpr int PIPE_THREADS = 256;
 constexpr int PIPE_TX = 32, PIPE_TY = 8;  // tile of the N, K, ADV items; LB items are 256 consecutive nodes of a plane
-constexpr int PIPE_RING = 6;              // planes per ring (the schedule keeps at most 4 live)
+// Planes per ring: just what the schedule keeps live plus one macro step of slack, so that the rings' footprint
+// in L2 stays small and a dead plane is overwritten while its lines are still resident (no write-back to HBM).
+constexpr int RING_N = 4, RING_GC = 3, RING_R = 4, RING_U = 4, RING_FZ = 3;
+constexpr int PIPE_RING_DOUBLES = 3 * RING_N + 4 * RING_GC + RING_R + 3 * RING_U + RING_FZ;  // per node of a plane
+// Macro step m holds N(zz = m - 2), LB(zz = m - 2 - LAG_LB), K(zz = m - 2 - LAG_K), ADV(zz = m - 2 - LAG_ADV).
+constexpr int LAG_K = 1, LAG_LB = 2, LAG_ADV = 4;
 enum { ST_N = 0, ST_LB = 1, ST_K = 2, ST_ADV = 3 };
 
 struct PipeArgs {
@@ -41,17 +46,17 @@ struct PipeArgs {
   const double* phi;  // phi(t), [nz][ny][nx]
   double* phi_new;    // phi(t+1)
   const double* tabs;
-  double* ring_n;     // [PIPE_RING][3][ny][nx]
-  double* ring_gc;    // [PIPE_RING][4][ny][nx]  g_x g_y g_z c
-  double* ring_r;     // [PIPE_RING][ny][nx]
-  double* ring_u;     // [PIPE_RING][3][ny][nx]
-  double* ring_fz;    // [PIPE_RING][ny][nx]     advective flux through the face (z, z+1)
+  double* ring_n;     // [RING_N][3][ny][nx]
+  double* ring_gc;    // [RING_GC][4][ny][nx]  g_x g_y g_z c
+  double* ring_r;     // [RING_R][ny][nx]
+  double* ring_u;     // [RING_U][3][ny][nx]
+  double* ring_fz;    // [RING_FZ][ny][nx]     advective flux through the face (z, z+1)
   int* ticket;        // one counter
   int* done;          // [4][nz + 4] completion counters, index zz + 2
   int tiles_x, tiles_y, tiles;  // tiles of PIPE_TX x PIPE_TY per plane
   int lb_items;                 // ceil(nx ny / 256)
   int per_macro;                // 3 tiles + lb_items
-  int total;                    // (nz + 5) per_macro
+  int total;                    // (nz + 3 + LAG_ADV) per_macro
 };
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
@@ -68,7 +73,8 @@ __device__ __forceinline__ int wrapg(int a, int n) {
   }
   return a;
 }
-__device__ __forceinline__ int ring_slot(int zz) { return (zz + 2) % PIPE_RING; }
+template <int R>
+__device__ __forceinline__ int ring_slot(int zz) { return (zz + 2) % R; }
 
 // 3 x 3 in-plane stencils on a row-major plane of pitch PX, p pointing at the (-1,-1) corner; W = (1,4,1)
 template <int PX>
@@ -132,7 +138,7 @@ __device__ __forceinline__ void stage_N(const PipeArgs& a, PipeSmem& S, int zz, 
     const double gy = (1.0 / 72.0) * st_SxDy<HX>(&S.n.Tz[ty][tx]);
     const double gz = (1.0 / 72.0) * st_SxSy<HX>(&S.n.Dz[ty][tx]);
     const double inv = 1.0 / (sqrt(fma(gx, gx, fma(gy, gy, gz * gz))) + 1e-12);  // R17
-    double* out = a.ring_n + (size_t)ring_slot(zz) * 3 * plane + (unsigned)y * (unsigned)G.nx + (unsigned)x;
+    double* out = a.ring_n + (size_t)ring_slot<RING_N>(zz) * 3 * plane + (unsigned)y * (unsigned)G.nx + (unsigned)x;
     out[0] = gx * inv;
     out[plane] = gy * inv;
     out[2 * plane] = gz * inv;
@@ -151,9 +157,9 @@ __device__ __forceinline__ void stage_K(const PipeArgs& a, PipeSmem& S, int zz, 
   const double* pm = a.phi + (size_t)wrap_dec(z, G.nz) * plane;
   const double* pc = a.phi + (size_t)z * plane;
   const double* pp = a.phi + (size_t)wrap_inc(z, G.nz) * plane;
-  const double* nm = a.ring_n + (size_t)ring_slot(zz - 1) * 3 * plane;
-  const double* nc = a.ring_n + (size_t)ring_slot(zz) * 3 * plane;
-  const double* np = a.ring_n + (size_t)ring_slot(zz + 1) * 3 * plane;
+  const double* nm = a.ring_n + (size_t)ring_slot<RING_N>(zz - 1) * 3 * plane;
+  const double* nc = a.ring_n + (size_t)ring_slot<RING_N>(zz) * 3 * plane;
+  const double* np = a.ring_n + (size_t)ring_slot<RING_N>(zz + 1) * 3 * plane;
   for (int e = tid; e < HX * HY; e += PIPE_THREADS) {
     const int j = e / HX, i = e - j * HX;
     const unsigned off = (unsigned)wrapg(y0 - 1 + j, G.ny) * (unsigned)G.nx + (unsigned)wrapg(x0 - 1 + i, G.nx);
@@ -184,12 +190,12 @@ __device__ __forceinline__ void stage_K(const PipeArgs& a, PipeSmem& S, int zz, 
     const double lap = 6.0 * (st_SxSy<HX>(&S.k.f[6][ty][tx]) * (1.0 / 216.0) - S.k.f[8][ty + 1][tx + 1]);  // R7
     const double gn = sqrt(fma(gx, gx, fma(gy, gy, gz * gz)));
     const unsigned o = (unsigned)y * (unsigned)G.nx + (unsigned)x;
-    double* gc = a.ring_gc + (size_t)ring_slot(zz) * 4 * plane + o;
+    double* gc = a.ring_gc + (size_t)ring_slot<RING_GC>(zz) * 4 * plane + o;
     gc[0] = gx;
     gc[plane] = gy;
     gc[2 * plane] = gz;
     gc[3 * plane] = -a.P.sig15w * kc * gn;  // F^s = c g (R8)
-    a.ring_r[(size_t)ring_slot(zz) * plane + o] = a.P.D * lap - a.P.kappa * dq;  // phi-only part of Eq. 3
+    a.ring_r[(size_t)ring_slot<RING_R>(zz) * plane + o] = a.P.D * lap - a.P.kappa * dq;  // phi-only part of Eq. 3
   }
 }
 
@@ -209,7 +215,7 @@ __device__ __forceinline__ void stage_LB(const PipeArgs& a, int zz, int item) {
   const unsigned k = (unsigned)z * plane + idx;
   double f[Q];
   pull27<ST>((const ST*)a.fin, G, nb, f);
-  const double* gc = a.ring_gc + (size_t)ring_slot(zz) * 4 * plane + idx;
+  const double* gc = a.ring_gc + (size_t)ring_slot<RING_GC>(zz) * 4 * plane + idx;
   const double g[3] = {__ldcg(gc), __ldcg(gc + plane), __ldcg(gc + 2 * plane)};
   const double c = __ldcg(gc + 3 * plane);
   const double phi0 = __ldg(a.phi + k);
@@ -219,7 +225,7 @@ __device__ __forceinline__ void stage_LB(const PipeArgs& a, int zz, int item) {
   body_force(P, a.tabs, x, y, z, Fb);
   accel_from_gc(P, M, g, c, phi0, Fb, true, A, rho);
   const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
-  double* uo = a.ring_u + (size_t)ring_slot(zz) * 3 * plane + idx;
+  double* uo = a.ring_u + (size_t)ring_slot<RING_U>(zz) * 3 * plane + idx;
   uo[0] = u[0];
   uo[plane] = u[1];
   uo[2 * plane] = u[2];
@@ -240,8 +246,8 @@ __device__ __forceinline__ void stage_ADV(const PipeArgs& a, PipeSmem& S, int zz
   const bool active = x < G.nx && y < G.ny;
   const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
   const unsigned own = (unsigned)wrapg(y, G.ny) * (unsigned)G.nx + (unsigned)wrapg(x, G.nx);
-  const double* uc = a.ring_u + (size_t)ring_slot(zz) * 3 * plane;
-  const double* uzp = a.ring_u + (size_t)ring_slot(zz + 1) * 3 * plane + 2 * plane;
+  const double* uc = a.ring_u + (size_t)ring_slot<RING_U>(zz) * 3 * plane;
+  const double* uzp = a.ring_u + (size_t)ring_slot<RING_U>(zz + 1) * 3 * plane + 2 * plane;
   auto zoff = [&](int k) { return (size_t)wrapg(z + k + G.nz, G.nz) * plane; };
   const size_t zo = (size_t)z * plane;
 
@@ -270,13 +276,13 @@ __device__ __forceinline__ void stage_ADV(const PipeArgs& a, PipeSmem& S, int zz
   S.a.phi[ty + 3][tx + 3] = w2;
   S.a.ux[ty][tx + 1] = __ldcg(uc + own);
   S.a.uy[ty + 1][tx] = __ldcg(uc + plane + own);
-  const double rr = __ldcg(a.ring_r + (size_t)ring_slot(zz) * plane + own);
+  const double rr = __ldcg(a.ring_r + (size_t)ring_slot<RING_R>(zz) * plane + own);
   double fz_lo;
   if (zz == 0) {  // the first plane of the sweep evaluates its lower face itself (same operations, same bits)
-    const double uzm = __ldcg(a.ring_u + (size_t)ring_slot(zz - 1) * 3 * plane + 2 * plane + own);
+    const double uzm = __ldcg(a.ring_u + (size_t)ring_slot<RING_U>(zz - 1) * 3 * plane + 2 * plane + own);
     fz_lo = face_flux(uzm, uz0, __ldg(a.phi + zoff(-3) + own), w0, w1, w2, w3, w4);
   } else {
-    fz_lo = __ldcg(a.ring_fz + (size_t)ring_slot(zz - 1) * plane + own);
+    fz_lo = __ldcg(a.ring_fz + (size_t)ring_slot<RING_FZ>(zz - 1) * plane + own);
   }
   __syncthreads();
   for (int e = tid; e < TY * (TX + 1); e += PIPE_THREADS) {  // x faces
@@ -297,18 +303,41 @@ __device__ __forceinline__ void stage_ADV(const PipeArgs& a, PipeSmem& S, int zz
     adv += S.a.fy[ty + 1][tx] - S.a.fy[ty][tx];
     adv += fz - fz_lo;
     __stcs(a.phi_new + zo + own, w2 + (-adv + rr));
-    a.ring_fz[(size_t)ring_slot(zz) * plane + own] = fz;
+    a.ring_fz[(size_t)ring_slot<RING_FZ>(zz) * plane + own] = fz;
   }
 }
 
 // ---------------------------------------------------------------------------------------------------- the kernel
-__device__ __forceinline__ void wait_done(const PipeArgs& a, int stage, int zz, int count) {
-  const int* p = a.done + stage * (a.P.G.nz + 4) + zz + 2;
-  while (ld_acquire(p) < count) __nanosleep(40);
+// j-th thing item (stage, zz) has to wait for: the counter index and the count it must reach.  First the data
+// dependencies, then the readers of the ring planes the item is about to overwrite.
+__device__ __forceinline__ bool pipe_dep(const PipeArgs& a, int stage, int zz, int j, int& idx, int& cnt) {
+  const int nz = a.P.G.nz, npos = nz + 4;
+  int st = -1, z = 0;
+  if (stage == ST_N) {  // readers of n(zz - RING_N): K(zz - RING_N - 1 .. zz - RING_N + 1)
+    if (j < 3) { st = ST_K; z = zz - RING_N - 1 + j; }
+  } else if (stage == ST_K) {
+    if (j < 3) { st = ST_N; z = zz - 1 + j; }
+    else if (j == 3) { st = ST_LB; z = zz - RING_GC; }  // reader of g,c(zz - RING_GC)
+    else if (j == 4) { st = ST_ADV; z = zz - RING_R; }  // reader of r(zz - RING_R)
+  } else if (stage == ST_LB) {
+    if (j == 0) { st = ST_K; z = zz; }
+    else if (j == 1 && zz - RING_U >= -1) { st = ST_ADV; z = max(zz - RING_U, 0); }  // readers of u(zz - RING_U): ADV(zz - RING_U - 1), ADV(zz - RING_U); ADV(0) reads u(-1)
+  } else {
+    if (j == 0) { st = ST_LB; z = zz; }
+    else if (j == 1) { st = ST_LB; z = zz + 1; }
+    else if (j == 2) { if (zz == 0) { st = ST_LB; z = -1; } else { st = ST_ADV; z = zz - 1; } }  // also frees fz(zz - RING_FZ)
+  }
+  if (st < 0) return false;
+  const bool exists = st == ST_N ? (z >= -2 && z <= nz + 1) : st == ST_ADV ? (z >= 0 && z <= nz - 1) : (z >= -1 && z <= nz);
+  if (!exists) return false;
+  idx = st * npos + z + 2;
+  cnt = st == ST_LB ? a.lb_items : a.tiles;
+  return true;
 }
 
 template <typename ST, int MINB>
 __global__ void __launch_bounds__(PIPE_THREADS, MINB) k_step_tp(const __grid_constant__ PipeArgs a) {
+  static_assert(RING_FZ >= 2 && RING_N >= 3 && RING_GC >= 1 && RING_R >= 1 && RING_U >= 2, "ring depths");
   __shared__ PipeSmem S;
   const int tid = threadIdx.x;
   const int nz = a.P.G.nz;
@@ -324,34 +353,19 @@ __global__ void __launch_bounds__(PIPE_THREADS, MINB) k_step_tp(const __grid_con
     int r = t - m * a.per_macro;
     int stage, zz;
     if (r < a.tiles) { stage = ST_N; zz = m - 2; }
-    else if ((r -= a.tiles) < a.lb_items) { stage = ST_LB; zz = m - 4; }
-    else if ((r -= a.lb_items) < a.tiles) { stage = ST_K; zz = m - 3; }
-    else { r -= a.tiles; stage = ST_ADV; zz = m - 5; }
+    else if ((r -= a.tiles) < a.lb_items) { stage = ST_LB; zz = m - 2 - LAG_LB; }
+    else if ((r -= a.lb_items) < a.tiles) { stage = ST_K; zz = m - 2 - LAG_K; }
+    else { r -= a.tiles; stage = ST_ADV; zz = m - 2 - LAG_ADV; }
     const bool valid = stage == ST_N ? (zz >= -2 && zz <= nz + 1)
                                      : stage == ST_ADV ? (zz >= 0 && zz <= nz - 1) : (zz >= -1 && zz <= nz);
     if (!valid) {
       __syncthreads();
       continue;
     }
-    if (tid == 0) {  // dependencies (smaller tickets only), then ring-slot reuse (always long satisfied, kept for safety)
-      if (stage == ST_N) {
-        for (int k = zz - PIPE_RING - 1; k <= zz - PIPE_RING + 1; ++k)  // the three readers of n(zz - PIPE_RING)
-          if (k >= -1 && k <= nz) wait_done(a, ST_K, k, a.tiles);
-      } else if (stage == ST_K) {
-        wait_done(a, ST_N, zz - 1, a.tiles);
-        wait_done(a, ST_N, zz, a.tiles);
-        wait_done(a, ST_N, zz + 1, a.tiles);
-        if (zz - PIPE_RING >= -1) wait_done(a, ST_LB, zz - PIPE_RING, a.lb_items);
-        if (zz - PIPE_RING >= 0) wait_done(a, ST_ADV, zz - PIPE_RING, a.tiles);
-      } else if (stage == ST_LB) {
-        wait_done(a, ST_K, zz, a.tiles);
-        if (zz - PIPE_RING + 1 >= 0) wait_done(a, ST_ADV, zz - PIPE_RING + 1, a.tiles);
-      } else {
-        wait_done(a, ST_LB, zz, a.lb_items);
-        wait_done(a, ST_LB, zz + 1, a.lb_items);
-        if (zz == 0) wait_done(a, ST_LB, -1, a.lb_items);
-        else wait_done(a, ST_ADV, zz - 1, a.tiles);
-      }
+    if (tid < 5) {  // each dependency is polled by its own thread: one L2 round trip when all are already satisfied
+      int idx, cnt;
+      if (pipe_dep(a, stage, zz, tid, idx, cnt))
+        while (ld_acquire(a.done + idx) < cnt) __nanosleep(40);
     }
     __syncthreads();
     if (stage == ST_N) stage_N(a, S, zz, r);

@@ -34,29 +34,55 @@ __device__ __forceinline__ double lattice_laplacian(V val) {
   return 6.0 * (acc * (1.0 / 216.0) - val(0, 0, 0));
 }
 
+// cp.async (LDGSTS) of one population from global memory into the issuing thread's own shared-memory slot, with an
+// L2 evict-first policy: the populations stream through once per step and must not displace phi, u, r in L2.
+__device__ __forceinline__ unsigned long long l2_evict_first_policy() {
+  unsigned long long p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+template <int BYTES>
+__device__ __forceinline__ void cp_async_pop(void* smem, const void* gmem, unsigned long long pol) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], %2, %3;" ::"r"(sa), "l"(gmem), "n"(BYTES), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_f64(double* smem, const double* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void cp_async_wait_but() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 // Shared-memory working set of k_lb_tp for one TX x TY column marching along z.
 //   The D3Q27 stencil weights factorise, w_i = W(cx) W(cy) W(cz) / 216 with W = (1,4,1), so every lattice stencil of
 //   PAPER.md:L104 is evaluated separably: a z combination per (x,y) column first (Sz = (1,4,1), Dz = (+1,0,-1)), then a
 //   3 x 3 stencil in the plane.  Same numbers as the 27-term sums up to rounding order.
-template <int TX, int TY>
+template <typename ST, int TX, int TY>
 struct GeoTile {
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
-  double raw[3][PY][PX];     // ring of raw phi planes zc-1, zc, zc+1
-  double Tz[PY][PX];         // Sz phi at plane zc
-  double Dz[PY][PX];         // Dz phi at plane zc
-  double nq[2][6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc (slot zc & 1), q = phi (1 - phi) n
-  double own[2][5][TY][TX];  // g_x g_y g_z |g| lap(phi) of plane zc at the tile's own nodes (slot zc & 1)
+  double raw[4][PY][PX];  // ring of raw phi planes zc-1, zc, zc+1 and zc+2 (landing, cp.async)
+  double Tz[PY][PX];      // Sz phi at plane zc
+  double Dz[PY][PX];      // Dz phi at plane zc
+  double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
+  ST fpop[Q][TX * TY];    // landing zone of the prefetched populations of the next plane: slot [i][tid] is thread tid's
 };
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
-// Iteration zc: stage phi(zc+1) -> Sz, Dz of plane zc | derive n, q, g, |g|, lap on plane zc | plane sums of plane zc,
-// then the node update of plane z = zc - 1, whose z combinations need planes zc-2 .. zc (carried in registers).
+// Iteration zc: stage phi(zc+1) -> Sz, Dz of plane zc | derive n, q (tile + 1) and g, |g|, lap (own node, kept in
+// registers) on plane zc | plane sums of plane zc, then the node update of plane z = zc - 1, whose z combinations need
+// planes zc-2 .. zc (carried in registers).
+// The 27 populations a thread pulls for plane z are fetched with cp.async into the thread's own shared-memory slots while
+// the block is still busy with plane z-1 and with the geometry of plane z: the HBM latency of the pull hides under the
+// fp64 work instead of stalling every warp at the top of the node update, and no register holds a load in flight.
 template <typename ST, int TX, int TY, int MINB>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
         double* __restrict__ uout, double* __restrict__ rout, const double* __restrict__ tabs, int lz) {
-  using T = GeoTile<TX, TY>;
+  using T = GeoTile<ST, TX, TY>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T& S = *reinterpret_cast<T*>(smem_raw);
   constexpr int NT = TX * TY;
@@ -70,6 +96,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const int x = x0 + tx, y = y0 + ty;
   const bool active = x < G.nx && y < G.ny;
   const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
+  const unsigned long long pol = l2_evict_first_policy();
 
   // rim item of the staging pass: the tid-th element of the PY x PX plane that is not an own node
   int r2 = -1;  // linear index j * PX + i in a phi plane
@@ -97,6 +124,28 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const unsigned yrow[3] = {(unsigned)wrap_dec(yw, G.ny) * (unsigned)G.nx, (unsigned)yw * (unsigned)G.nx,
                             (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx};
 
+  // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1), as 27 asynchronous copies
+  auto prefetch_pull = [&](int z) {
+    const unsigned zr[3] = {(unsigned)wrap_dec(z, G.nz) * plane, (unsigned)z * plane, (unsigned)wrap_inc(z, G.nz) * plane};
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      const unsigned src = zr[1 - cz_of(i)] + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)];
+      cp_async_pop<(int)sizeof(ST)>(&S.fpop[i][tid], fin + (size_t)i * G.n + src, pol);
+    }
+    cp_async_commit();
+  };
+  // Per-thread cp.async groups alternate phi plane | populations, every thread commits both in every iteration (an
+  // empty group where it has nothing to fetch), so "all but the newest group" is always the one needed next.
+  // phi(zc+2) lands in the 4th ring plane one iteration before it is combined: its latency hides under plane zc.
+  {
+    const double* s2 = phi + (size_t)pmod(z0, G.nz) * plane;
+    cp_async_f64(&S.raw[2][0][0] + o2, s2 + o2off);
+    if (r2 >= 0) cp_async_f64(&S.raw[2][0][0] + r2, s2 + r2off);
+    cp_async_commit();
+  }
+  if (active) prefetch_pull(z0);
+  else cp_async_commit();
+
   // stage raw phi planes z0-2 and z0-1
   {
     const double* s0 = phi + (size_t)pmod(z0 - 2, G.nz) * plane;
@@ -112,36 +161,60 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   }
   double an0 = 0.0, an1 = 0.0, bn0 = 0.0, bn1 = 0.0;  // plane sums of n at planes zc-2, zc-1
   double aq0 = 0.0, aq1 = 0.0, bq0 = 0.0, bq1 = 0.0;  // plane sums of q
+  double gp[3] = {0.0, 0.0, 0.0}, gnp = 0.0, lapp = 0.0;  // g, |g|, lap phi of the own node at plane zc-1
+  // x- and y-dependent parts of the body force are fixed along the march (R20)
+  double fsx = 0.0, fcx = 0.0, fsy = 0.0, fcy = 0.0;
+  if (P.force_type != 0) {
+    fsx = __ldg(tabs + xw); fcx = __ldg(tabs + G.nx + xw);
+    fsy = __ldg(tabs + 2 * G.nx + yw); fcy = __ldg(tabs + 2 * G.nx + G.ny + yw);
+  }
   __syncthreads();
 
   for (int zc = z0 - 1; zc <= z1; ++zc) {
     const int it = zc - (z0 - 1);  // 0, 1, 2, ...
-    // ---- stage phi(zc+1); z combinations of plane zc
+    // body-force density of the node updated in this iteration (plane zc-1), R20; loaded before the barriers
+    double Fb[3] = {0.0, 0.0, 0.0};
+    if (P.force_type != 0 && zc > z0 - 1) {
+      const double fsz = __ldg(tabs + 2 * (G.nx + G.ny) + (zc - 1)), fcz = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + (zc - 1));
+      if (P.force_type == 1) {  // ABC
+        Fb[0] = P.force_amp * (fsz + fcy);
+        Fb[1] = P.force_amp * (fsx + fcz);
+        Fb[2] = P.force_amp * (fsy + fcx);
+      } else {  // sine variant of BASELINE config 2
+        Fb[0] = P.force_amp * fsy;
+        Fb[1] = P.force_amp * fsz;
+        Fb[2] = P.force_amp * fsx;
+      }
+    }
+    // ---- phi(zc+1) has landed (this thread's own elements); fetch phi(zc+2); z combinations of plane zc
     {
-      const double* src = phi + (size_t)pmod(zc + 1, G.nz) * plane;
-      const double* rm = &S.raw[it % 3][0][0];        // plane zc-1
-      const double* rc = &S.raw[(it + 1) % 3][0][0];  // plane zc
-      double* rp = &S.raw[(it + 2) % 3][0][0];        // plane zc+1
+      cp_async_wait_but<1>();
+      const double* rm = &S.raw[it & 3][0][0];        // plane zc-1
+      const double* rc = &S.raw[(it + 1) & 3][0][0];  // plane zc
+      const double* rp = &S.raw[(it + 2) & 3][0][0];  // plane zc+1
+      double* rn = &S.raw[(it + 3) & 3][0][0];        // plane zc+2, last read (as plane zc-2) by this same thread
+      if (zc < z1) {
+        const double* src = phi + (size_t)pmod(zc + 2, G.nz) * plane;
+        cp_async_f64(rn + o2, src + o2off);
+        if (r2 >= 0) cp_async_f64(rn + r2, src + r2off);
+      }
+      cp_async_commit();
       double* tz = &S.Tz[0][0];
       double* dz = &S.Dz[0][0];
-      const double v = __ldg(src + o2off);
-      const double m = rm[o2];
-      rp[o2] = v;
+      const double v = rp[o2], m = rm[o2];
       tz[o2] = fma(4.0, rc[o2], m + v);
       dz[o2] = v - m;
       if (r2 >= 0) {
-        const double v2 = __ldg(src + r2off);
-        const double m2 = rm[r2];
-        rp[r2] = v2;
+        const double v2 = rp[r2], m2 = rm[r2];
         tz[r2] = fma(4.0, rc[r2], m2 + v2);
         dz[r2] = v2 - m2;
       }
     }
     __syncthreads();
-    // ---- derive n, q (tile + 1 rim) and g, |g|, lap (own nodes) on plane zc           PAPER.md:L61, L104; R17
+    // ---- derive n, q (tile + 1 rim) and g, |g|, lap (own node) on plane zc           PAPER.md:L61, L104; R17
+    double gc[3], gnc, lapc;
     {
-      const int slot = zc & 1;
-      const double* rc = &S.raw[(it + 1) % 3][0][0];
+      const double* rc = &S.raw[(it + 1) & 3][0][0];
       auto derive = [&](int j, int i, bool own_node) {  // (j, i) in the NY x NX plane; centre (j+1, i+1) in a phi plane
         const double* t = &S.Tz[j][i];
         const double* d = &S.Dz[j][i];
@@ -159,20 +232,17 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const double ph = rc[(j + 1) * PX + (i + 1)];
         const double pq = ph * (1.0 - ph);
         const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
-        S.nq[slot][0][j][i] = nx_;
-        S.nq[slot][1][j][i] = ny_;
-        S.nq[slot][2][j][i] = nz_;
-        S.nq[slot][3][j][i] = pq * nx_;
-        S.nq[slot][4][j][i] = pq * ny_;
-        S.nq[slot][5][j][i] = pq * nz_;
+        S.nq[0][j][i] = nx_;
+        S.nq[1][j][i] = ny_;
+        S.nq[2][j][i] = nz_;
+        S.nq[3][j][i] = pq * nx_;
+        S.nq[4][j][i] = pq * ny_;
+        S.nq[5][j][i] = pq * nz_;
         if (own_node) {
           const double s0 = fma(4.0, t01, t00 + t02), s1 = fma(4.0, t11, t10 + t12), s2 = fma(4.0, t21, t20 + t22);
-          const double lap = 6.0 * (fma(4.0, s1, s0 + s2) * (1.0 / 216.0) - ph);  // R7
-          S.own[slot][0][j - 1][i - 1] = gx;
-          S.own[slot][1][j - 1][i - 1] = gy;
-          S.own[slot][2][j - 1][i - 1] = gz;
-          S.own[slot][3][j - 1][i - 1] = gn;
-          S.own[slot][4][j - 1][i - 1] = lap;
+          gc[0] = gx; gc[1] = gy; gc[2] = gz;
+          gnc = gn;
+          lapc = 6.0 * (fma(4.0, s1, s0 + s2) * (1.0 / 216.0) - ph);  // R7
         }
       };
       derive(ty + 1, tx + 1, true);
@@ -182,12 +252,11 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     // ---- plane sums of plane zc at the own node:  a = Dx Sy v_x + Sx Dy v_y,  b = Sx Sy v_z
     double an2, bn2, aq2, bq2;
     {
-      const int slot = zc & 1;
       constexpr int NX = T::NX;
       auto plane_sums = [&](int c0, double& a, double& b) {
-        const double* vx = &S.nq[slot][c0][ty][tx];
-        const double* vy = &S.nq[slot][c0 + 1][ty][tx];
-        const double* vz = &S.nq[slot][c0 + 2][ty][tx];
+        const double* vx = &S.nq[c0][ty][tx];
+        const double* vy = &S.nq[c0 + 1][ty][tx];
+        const double* vz = &S.nq[c0 + 2][ty][tx];
         const double ax = fma(4.0, vx[NX + 2] - vx[NX], (vx[2] - vx[0]) + (vx[2 * NX + 2] - vx[2 * NX]));
         const double ay = fma(4.0, vy[2 * NX + 1] - vy[1], (vy[2 * NX] - vy[0]) + (vy[2 * NX + 2] - vy[2]));
         a = ax + ay;
@@ -200,45 +269,33 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       plane_sums(3, aq2, bq2);
     }
     const int z = zc - 1;
+    if (!(z >= z0 && active)) cp_async_commit();
     if (z >= z0 && active) {
+      // a1-a2: the pulled populations have landed in this thread's slots; moments, then refill the slots for plane z+1
+      cp_async_wait_but<1>();
+      Moments M;
+      moments_of([&](int i) { return Pop<ST>::from_storage(S.fpop[i][tid], i); }, M);
+      if (z + 1 < z1) prefetch_pull(z + 1);
+      else cp_async_commit();
       // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
       const double kc = (1.0 / 72.0) * (fma(4.0, an1, an0 + an2) + (bn2 - bn0));
       const double divq = (1.0 / 72.0) * (fma(4.0, aq1, aq0 + aq2) + (bq2 - bq0));
-      const int so = z & 1;
-      const double g[3] = {S.own[so][0][ty][tx], S.own[so][1][ty][tx], S.own[so][2][ty][tx]};
-      const double gn = S.own[so][3][ty][tx];
-      const double lap = S.own[so][4][ty][tx];
-      const double phi0 = S.raw[it % 3][ty + 2][tx + 2];  // plane zc-1 = z
+      const double phi0 = S.raw[it & 3][ty + 2][tx + 2];  // plane zc-1 = z
 
       const unsigned k = (unsigned)z * plane + yrow[1] + (unsigned)xs[1];
-      rout[k] = P.D * lap - P.kappa * divq;  // phi-only part of Eq. 3
+      rout[k] = P.D * lapp - P.kappa * divq;  // phi-only part of Eq. 3
 
-      // a1: pull-stream
-      Nbr nb;
-      nb.x[0] = xs[0]; nb.x[1] = xs[1]; nb.x[2] = xs[2];
-      {
-        const unsigned zr[3] = {(unsigned)wrap_dec(z, G.nz) * plane, (unsigned)z * plane,
-                                (unsigned)wrap_inc(z, G.nz) * plane};
-#pragma unroll
-        for (int a = 0; a < 3; ++a)
-#pragma unroll
-          for (int b = 0; b < 3; ++b) nb.row[a][b] = zr[a] + yrow[b];
-      }
-      double f[Q];
-      pull27<ST>(fin, G, nb, f);
-      Moments M;
-      moments_of(f, M);
-      double Fb[3], A[3], rho;
-      body_force(P, tabs, x, y, z, Fb);
-      accel_from_geometry(P, M, g, gn, kc, phi0, Fb, true, A, rho);
+      double A[3], rho;
+      accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, true, A, rho);
       const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
       uout[k] = u[0];
       uout[G.n + k] = u[1];
       uout[2u * G.n + k] = u[2];
-      collide_store<ST>(P, M, u, A, f, fout, k);
+      collide_store<ST>(P, M, u, A, fout, k);
     }
     an0 = an1; an1 = an2; bn0 = bn1; bn1 = bn2;
     aq0 = aq1; aq1 = aq2; bq0 = bq1; bq1 = bq2;
+    gp[0] = gc[0]; gp[1] = gc[1]; gp[2] = gc[2]; gnp = gnc; lapp = lapc;
   }
 }
 
