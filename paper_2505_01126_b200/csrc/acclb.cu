@@ -116,7 +116,7 @@ __device__ __forceinline__ void accel_from_gc(const KP& P, const Moments& M, con
     F[1] -= P.visc_pref * (sxy * dr[0] + syy * dr[1] + syz * dr[2]);
     F[2] -= P.visc_pref * (sxz * dr[0] + syz * dr[1] + szz * dr[2]);
   }
-  const double ir = 1.0 / rho;
+  const double ir = div_pos(1.0, rho);
   A[0] = F[0] * ir; A[1] = F[1] * ir; A[2] = F[2] * ir;
 }
 
@@ -564,10 +564,17 @@ static int launch_lb_tp(accLB_ctx* s, int c, int d) {
 }
 
 static int launch_advect(accLB_ctx* s, int c, int d) {
+  using T = AdvTile<ADV_TX, ADV_TY>;
+  auto kern = k_advect<ADV_TX, ADV_TY>;
+  static thread_local int configured_device = -1;
+  if (configured_device != s->prm.device) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
+    configured_device = s->prm.device;
+  }
   const int lz = planes_per_block(s->nx, s->ny, s->nz, ADV_TX, ADV_TY);
   const dim3 grid((s->nx + ADV_TX - 1) / ADV_TX, (s->ny + ADV_TY - 1) / ADV_TY, (s->nz + lz - 1) / lz);
   LaunchScope ls(s, KIND_AC);
-  k_advect<ADV_TX, ADV_TY><<<grid, ADV_TX * ADV_TY, 0, s->stream>>>(s->kp, s->phi[c], s->u, s->r, s->phi[d], lz);
+  kern<<<grid, ADV_TX * ADV_TY, sizeof(T), s->stream>>>(s->kp, s->phi[c], s->u, s->r, s->phi[d], lz);
   return ACCLB_OK;
 }
 

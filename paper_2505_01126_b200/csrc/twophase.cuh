@@ -228,7 +228,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const double r2_ = fma(4.0, d[2 * PX + 1], d[2 * PX] + d[2 * PX + 2]);
         const double gz = (1.0 / 72.0) * fma(4.0, r1, r0 + r2_);
         const double gn = sqrt(fma(gx, gx, fma(gy, gy, gz * gz)));
-        const double inv = 1.0 / (gn + 1e-12);
+        const double inv = div_pos(1.0, gn + 1e-12);
         const double ph = rc[(j + 1) * PX + (i + 1)];
         const double pq = ph * (1.0 - ph);
         const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
@@ -300,31 +300,37 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
 }
 
 // ---------------------------------------------------------------------------------------------------- advection
+// Shared memory of k_advect.  Everything a plane needs is fetched with cp.async one plane ahead (no register holds a
+// load in flight); buffers that only their owner thread touches (col, uz, r) need no barrier.
 template <int TX, int TY>
 struct AdvTile {
-  double phi[TY + 6][TX + 6];  // plane z with halo 3 along x and y (corners unused)
-  double ux[TY][TX + 2];       // u_x with halo 1 along x
-  double uy[TY + 2][TX];       // u_y with halo 1 along y
-  double fx[TY][TX + 1];       // flux through the x face between tile columns i-1 and i
-  double fy[TY + 1][TX];       // flux through the y face between tile rows j-1 and j
+  double phi[2][TY + 6][TX + 6];  // plane z (ping-pong) with halo 3 along x and y (corners unused)
+  double ux[2][TY][TX + 2];       // u_x with halo 1 along x
+  double uy[2][TY + 2][TX];       // u_y with halo 1 along y
+  double fx[TY][TX + 1];          // flux through the x face between tile columns i-1 and i
+  double fy[TY + 1][TX];          // flux through the y face between tile rows j-1 and j
+  double col[2][TX * TY];         // landing slot of the thread's own phi(z+3) (ping-pong); the window lives in registers
+  double uz[2][TX * TY];          // landing slot of the thread's own u_z(z+1)
+  double r[2][TX * TY];           // r = D lap phi - kappa div q of planes z, z+1
 };
 
 template <int TX, int TY>
-__global__ void __launch_bounds__(TX * TY)
+__global__ void __launch_bounds__(TX * TY, 4)
 k_advect(KP P, const double* __restrict__ phi, const double* __restrict__ u, const double* __restrict__ r,
          double* __restrict__ phi_new, int lz) {
   using T = AdvTile<TX, TY>;
-  __shared__ T S2[2];  // ping-pong over z so that two barriers per plane suffice
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T& S = *reinterpret_cast<T*>(smem_raw);
   constexpr int NT = TX * TY;
-  static_assert(6 * (TX + TY) <= NT && 2 * (TX + TY) <= NT, "one halo element per thread");
+  static_assert(TX == 32 && TY >= 8 && 6 * (TX + TY) <= NT && 2 * (TX + TY) <= NT, "one warp per tile row, one halo element per thread");
   const Grid& G = P.G;
   const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * lz;
   const int z1 = min(z0 + lz, G.nz);
   const int x = x0 + tx, y = y0 + ty;
   const bool active = x < G.nx && y < G.ny;
-  const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
-  const unsigned n = G.n;
+  const size_t plane = (size_t)G.nx * (size_t)G.ny;
+  const size_t n = G.n;
   const unsigned own = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
 
   // phi halo element of this thread (tid < 6 (TX + TY)): rows above/below first, then columns left/right
@@ -342,60 +348,86 @@ k_advect(KP P, const double* __restrict__ phi, const double* __restrict__ u, con
   if (hj >= 0) hoff = (unsigned)pmod(y0 - 3 + hj, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 3 + hi, G.nx);
   // velocity halo element (tid < 2 (TX + TY)): u_y rows -1, TY ; u_x columns -1, TX
   int vkind = 0, vj = 0, vi = 0;  // 1: uy, 2: ux
-  unsigned voff = 0;
+  size_t voff = 0;
   if (tid < 2 * TX) {
     vkind = 1;
     vj = tid < TX ? 0 : TY + 1;
     vi = tid % TX;
-    voff = n + (unsigned)pmod(y0 - 1 + vj, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 + vi, G.nx);
+    voff = n + (size_t)pmod(y0 - 1 + vj, G.ny) * (size_t)G.nx + (size_t)pmod(x0 + vi, G.nx);
   } else if (tid < 2 * (TX + TY)) {
     const int e = tid - 2 * TX;
     vkind = 2;
     vj = e / 2;
     vi = (e & 1) ? TX + 1 : 0;
-    voff = (unsigned)pmod(y0 + vj, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 1 + vi, G.nx);
+    voff = (size_t)pmod(y0 + vj, G.ny) * (size_t)G.nx + (size_t)pmod(x0 - 1 + vi, G.nx);
   }
 
+  // asynchronous fetch of what plane zp needs on top of the rings: its tile of phi, u_x, u_y with halos, and r
+  auto fetch_plane = [&](int b, int zp) {  // zp already wrapped
+    const size_t zo = (size_t)zp * plane;
+    cp_async_f64(&S.phi[b][ty + 3][tx + 3], phi + zo + own);
+    cp_async_f64(&S.ux[b][ty][tx + 1], u + zo + own);
+    cp_async_f64(&S.uy[b][ty + 1][tx], u + n + zo + own);
+    cp_async_f64(&S.r[b][tid], r + zo + own);
+    if (hj >= 0) cp_async_f64(&S.phi[b][hj][hi], phi + zo + hoff);
+    if (vkind == 1) cp_async_f64(&S.uy[b][vj][vi], u + zo + voff);
+    else if (vkind == 2) cp_async_f64(&S.ux[b][vj][vi], u + zo + voff);
+  };
+  // what the first plane needs, fetched asynchronously: its tile, and the newest members of the two z windows
   auto zoff = [&](int zz) { return (size_t)pmod(zz, G.nz) * plane; };
-  // column window w[j] = phi(z - 2 + j), j = 0..5, of the z face between z and z + 1
-  double w0 = __ldg(phi + zoff(z0 - 3) + own), w1 = __ldg(phi + zoff(z0 - 2) + own), w2 = __ldg(phi + zoff(z0 - 1) + own);
-  double w3 = __ldg(phi + zoff(z0) + own), w4 = __ldg(phi + zoff(z0 + 1) + own), w5 = __ldg(phi + zoff(z0 + 2) + own);
-  double uz0 = __ldg(u + 2u * n + zoff(z0 - 1) + own), uz1 = __ldg(u + 2u * n + zoff(z0) + own);
-  double fz_prev = face_flux(uz0, uz1, w0, w1, w2, w3, w4, w5);  // face (z0 - 1, z0)
+  cp_async_f64(&S.col[0][tid], phi + zoff(z0 + 3) + own);
+  cp_async_f64(&S.uz[0][tid], u + 2 * n + zoff(z0 + 1) + own);
+  fetch_plane(0, pmod(z0, G.nz));
+  cp_async_commit();
+  // column window w[j] = phi(z - 2 + j), j = 0..5, of the z face between z and z + 1; here still one plane behind
+  double w0, w1 = __ldg(phi + zoff(z0 - 2) + own), w2 = __ldg(phi + zoff(z0 - 1) + own), w3 = __ldg(phi + zoff(z0) + own);
+  double w4 = __ldg(phi + zoff(z0 + 1) + own), w5 = __ldg(phi + zoff(z0 + 2) + own);
+  double uz0, uz1 = __ldg(u + 2 * n + zoff(z0) + own);
+  double fz_prev = face_flux(__ldg(u + 2 * n + zoff(z0 - 1) + own), uz1, __ldg(phi + zoff(z0 - 3) + own), w1, w2, w3, w4, w5);  // face (z0 - 1, z0)
+  int zp1 = pmod(z0 + 1, G.nz), zp2 = pmod(z0 + 2, G.nz), zp4 = pmod(z0 + 4, G.nz);
 
   for (int z = z0; z < z1; ++z) {
-    T& S = S2[(z - z0) & 1];
-    const size_t zo = zoff(z);
+    const int b = (z - z0) & 1;
+    cp_async_wait_all();
+    __syncthreads();  // plane z is in shared memory; the x / y fluxes of plane z-1 have been consumed
     w0 = w1; w1 = w2; w2 = w3; w3 = w4; w4 = w5;
-    w5 = __ldg(phi + zoff(z + 3) + own);
+    w5 = S.col[b][tid];
     uz0 = uz1;
-    uz1 = __ldg(u + 2u * n + zoff(z + 1) + own);
-    S.phi[ty + 3][tx + 3] = w2;
-    S.ux[ty][tx + 1] = __ldg(u + zo + own);
-    S.uy[ty + 1][tx] = __ldg(u + n + zo + own);
-    if (hj >= 0) S.phi[hj][hi] = __ldg(phi + zo + hoff);
-    if (vkind == 1) S.uy[vj][vi] = __ldg(u + zo + voff);
-    else if (vkind == 2) S.ux[vj][vi] = __ldg(u + zo + voff);
-    const double rr = active ? __ldg(r + zo + own) : 0.0;
-    __syncthreads();
-    for (int e = tid; e < TY * (TX + 1); e += NT) {  // x faces
-      const int j = e / (TX + 1), i = e % (TX + 1);
-      const double* p = &S.phi[j + 3][i];  // p[0..5] = phi at tile columns i-3 .. i+2 = L-2 .. L+3 with L = i-1
-      S.fx[j][i] = face_flux(S.ux[j][i], S.ux[j][i + 1], p[0], p[1], p[2], p[3], p[4], p[5]);
+    uz1 = S.uz[b][tid];
+    if (z + 1 < z1) {  // fetch plane z+1
+      cp_async_f64(&S.col[b ^ 1][tid], phi + (size_t)zp4 * plane + own);  // phi(z+4)
+      cp_async_f64(&S.uz[b ^ 1][tid], u + 2 * n + (size_t)zp2 * plane + own);  // u_z(z+2)
+      fetch_plane(b ^ 1, zp1);
+      cp_async_commit();
+      zp1 = wrap_inc(zp1, G.nz); zp2 = wrap_inc(zp2, G.nz); zp4 = wrap_inc(zp4, G.nz);
     }
-    for (int e = tid; e < (TY + 1) * TX; e += NT) {  // y faces
-      const int j = e / TX, i = e % TX;
-      S.fy[j][i] = face_flux(S.uy[j][i], S.uy[j + 1][i], S.phi[j][i + 3], S.phi[j + 1][i + 3], S.phi[j + 2][i + 3],
-                             S.phi[j + 3][i + 3], S.phi[j + 4][i + 3], S.phi[j + 5][i + 3]);
+    {  // x face between tile columns tx and tx+1; one warp per tile row
+      const double* p = &S.phi[b][ty + 3][tx + 1];  // phi at tile columns tx-2 .. tx+3
+      S.fx[ty][tx + 1] = face_flux(S.ux[b][ty][tx + 1], S.ux[b][ty][tx + 2], p[0], p[1], p[2], p[3], p[4], p[5]);
+    }
+    {  // y face between tile rows ty and ty+1
+      const double(*q)[TX + 6] = S.phi[b];
+      S.fy[ty + 1][tx] = face_flux(S.uy[b][ty + 1][tx], S.uy[b][ty + 2][tx], q[ty + 1][tx + 3], q[ty + 2][tx + 3], q[ty + 3][tx + 3],
+                                   q[ty + 4][tx + 3], q[ty + 5][tx + 3], q[ty + 6][tx + 3]);
+    }
+    if (ty == 3 && tx < TY) {  // the TY faces on the tile's left edge
+      const double* p = &S.phi[b][tx + 3][0];
+      S.fx[tx][0] = face_flux(S.ux[b][tx][0], S.ux[b][tx][1], p[0], p[1], p[2], p[3], p[4], p[5]);
+    }
+    if (ty == TY - 1) {  // the TX faces on the tile's lower edge
+      const double(*q)[TX + 6] = S.phi[b];
+      S.fy[0][tx] = face_flux(S.uy[b][0][tx], S.uy[b][1][tx], q[0][tx + 3], q[1][tx + 3], q[2][tx + 3], q[3][tx + 3], q[4][tx + 3],
+                              q[5][tx + 3]);
     }
     const double fz = face_flux(uz0, uz1, w0, w1, w2, w3, w4, w5);  // face (z, z + 1)
+    const double rr = S.r[b][tid];
     __syncthreads();
     if (active) {
       double adv = 0.0;
       adv += S.fx[ty][tx + 1] - S.fx[ty][tx];
       adv += S.fy[ty + 1][tx] - S.fy[ty][tx];
       adv += fz - fz_prev;
-      phi_new[zo + own] = w2 + (-adv + rr);
+      __stcs(phi_new + (size_t)z * plane + own, w2 + (-adv + rr));
     }
     fz_prev = fz;
   }
