@@ -299,6 +299,20 @@ def roofline_of(meas, steps, fp32):
     return r
 
 
+def max_over_ranks(values, device=None):
+    """Element-wise maximum of `values` over all ranks of the default process group (the values themselves when
+    torch.distributed is not initialised).  The N > 1 path of this repo is "replicas only": no data-path collective,
+    this reduction of the device-timed milliseconds is the only exchange."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return list(values)
+    t = torch.tensor(list(values), dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
 def run_cuda(args):
     import torch
 
@@ -324,13 +338,8 @@ def run_cuda(args):
     cfg = make_workload(args.workload, args.n)
     meas = measure_cuda(cfg, args.steps, args.warmup, local_rank=local_rank, world=world, fp32=bool(args.fp32),
                         e2e=not args.no_e2e, variant=args.variant, barrier=barrier)
-    ms, e2e_ms = meas["ms"], meas.get("e2e", {}).get("ms", 0.0)
-    if world > 1:  # replicas only: every rank ran the same-sized independent problem; time = max over ranks
-        import torch.distributed as dist
-
-        t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=f"cuda:{local_rank}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms = t.tolist()
+    # replicas only: every rank ran the same-sized independent problem; time = max over ranks
+    ms, e2e_ms = max_over_ranks([meas["ms"], meas.get("e2e", {}).get("ms", 0.0)], f"cuda:{local_rank}" if world > 1 else None)
     if rank != 0:
         if world > 1:
             torch.distributed.destroy_process_group()
@@ -408,7 +417,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", choices=("cuda", "reference"), default="cuda")
     ap.add_argument("--workload", choices=sorted(WORKLOADS), default="bubbly")
-    ap.add_argument("--n", type=int, default=512, help="grid edge (default: the 512^3 the metric is quoted on)")
+    ap.add_argument("--n", "--grid", dest="n", type=int, default=512, help="grid edge (default: the 512^3 the metric is quoted on)")
     ap.add_argument("--fp32", type=int, default=0, help="1: fp32 population storage (arithmetic stays fp64)")
     ap.add_argument("--variant", type=int, default=None, help="kernel variant (accLB_set_variant), default = best")
     ap.add_argument("--no-e2e", action="store_true")

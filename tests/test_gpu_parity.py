@@ -319,3 +319,44 @@ def test_non_default_stream(acclb):
     ref.step(20)
     for x, y in zip(got, ref.moments()[:2]):
         assert torch.equal(x, y.cpu())
+
+
+# ---------------------------------------------------------------------------------------------- full size, sampled
+def test_config4_full_size_512_sampled_against_oracle(acclb):
+    """BASELINE config 4 at its full size (512^3, 60 bubbles), in the launch configuration bench.py times (default
+    variant, default stream): after k steps every node of three 44^3 sub-boxes (one wrapping the periodic corner, two
+    cutting through bubble interfaces) is compared with the oracle run on that periodic sub-box, whose interior is
+    exact beyond a rim of 3k + 2 nodes (tests/test_oracle_physics.py::test_subbox_evaluation_matches_full_box_interior).
+    Plus the properties that hold at any size: sum p* and sum phi conserved."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs about 80 GB of free device memory")
+    n, s, k = 512, 44, 3
+    cfg = wl.make_config("bubbly", n=n)
+    sim = gpu_sim(acclb, cfg)
+    d0 = sim.diagnostics()
+    sim.step(k)
+    rho, u, phi = (t.cpu().numpy() for t in sim.moments())
+    d1 = sim.diagnostics()
+    assert d1["step"] == k
+    assert abs(d1["sum_phi"] - d0["sum_phi"]) <= 1e-12 * d0["sum_phi"]
+    assert abs(d1["sum_pstar"] - d0["sum_pstar"]) <= 1e-12 * n ** 3
+    centres = wl.bubble_centres(n, 60)
+    origins = [(n - 20, n - 9, n - 30),
+               tuple(int(c) - s // 2 for c in centres[0]),                      # box centred on a bubble
+               (int(centres[7][0]) + 16 - s // 2, int(centres[7][1]) - s // 2, int(centres[7][2]) - s // 2)]  # on its rim
+    rim = 3 * k + 2
+    inner = (slice(rim, s - rim),) * 3
+    seen_interface = False
+    for org in origins:
+        o = oracle.Oracle(s, s, s, **cfg["params"], force_period=(n, n, n), force_origin=org)
+        o.init(wl.subbox(cfg["rho"], org, s), wl.subbox(cfg["u"], org, s), wl.subbox(cfg["phi"], org, s))
+        o.step(k)
+        ro, uo, po = o.moments()
+        o.close()
+        for name, a, b in (("rho", rho, ro), ("u", u, uo), ("phi", phi, po)):
+            diff = np.abs(wl.subbox(a, org, s)[..., inner[0], inner[1], inner[2]] - b[..., inner[0], inner[1], inner[2]]).max()
+            assert diff <= TOL, (org, name, diff)
+        pin = po[inner]
+        seen_interface |= bool(((pin > 0.1) & (pin < 0.9)).any())
+    assert seen_interface, "no sampled box cut through an interface"
