@@ -63,7 +63,7 @@ typedef struct {
 } accLB_params;
 
 /* Bytes of device workspace accLB_create needs for this grid and these parameters; 0 on invalid arguments
- * (nx, ny, nz >= 4, nx even, nx*ny*nz < 2^31, tau > 0.5, two_phase: rho_l, rho_g > 0, width > 0). */
+ * (nx, ny, nz >= 4, nx even, nx*ny*nz < 2^31, 27*nx*ny < 2^32, tau > 0.5, two_phase: rho_l, rho_g > 0, width > 0). */
 size_t accLB_workspace_bytes(int nx, int ny, int nz, const accLB_params* params);
 
 /* Create a context on `workspace` (DEVICE pointer, caller-owned, 256-byte aligned, >= workspace_bytes).

@@ -7,7 +7,7 @@
 //                                                                                     PAPER.md:L75-92 (Eqs. 4-7)
 //   k_allen_cahn (two-phase) conservative Allen-Cahn, flux-form WENO5 + lattice stencils, forward Euler (a8)
 //                                                                                     PAPER.md:L61-67 (Eq. 3)
-// State: post-collision, not yet streamed populations f*_i(x) in SoA [i][z][y][x], double-buffered (A/B), so the
+// State: post-collision, not yet streamed populations f*_i(x) in SoA [z][i][y][x], double-buffered (A/B), so the
 // pull f_i(x,t) = f*_i(x - c_i, t-1) reads shifted rows and every store is aligned; phi double-buffered.
 // No CPU fallback, no library kernels: everything the path computes runs in the kernels of this file.
 #include <cuda_runtime.h>
@@ -87,9 +87,11 @@ __device__ __forceinline__ void body_force(const KP& P, const double* __restrict
 // a1: pull-stream.  f_i(x,t) = f*_i(x - c_i, t-1), periodic wrap.   PAPER.md:L75/L85 (LHS of Eqs. 4, 6), L118
 template <typename ST>
 __device__ __forceinline__ void pull27(const ST* __restrict__ fin, const Grid& G, const Nbr& nb, double (&f)[Q]) {
+  const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
+  const ST* slab[3] = {pop_slab(fin, G, nb.z[0]), pop_slab(fin, G, nb.z[1]), pop_slab(fin, G, nb.z[2])};
 #pragma unroll
   for (int i = 0; i < Q; ++i)
-    f[i] = Pop<ST>::load(fin + (size_t)i * G.n + nb.at(-cz_of(i), -cy_of(i), -cx_of(i)), i);
+    f[i] = Pop<ST>::load(slab[1 - cz_of(i)] + ((unsigned)i * plane + nb.yr[1 - cy_of(i)] + (unsigned)nb.x[1 - cx_of(i)]), i);
 }
 
 // a4-a5: total force, acceleration A = F / rho (R3) and density at a node from its interface geometry.
@@ -168,7 +170,7 @@ __device__ __forceinline__ void hermite_coeff(const Moments& M, const double (&u
 // population (see hermite2_populations), aligned store of f*_i(x) into the other buffer.
 template <typename ST>
 __device__ __forceinline__ void collide_store(const KP& P, const Moments& M, const double (&u)[3], const double (&A)[3],
-                                              double (&f)[Q], ST* __restrict__ fout, unsigned k) {
+                                              double (&f)[Q], ST* __restrict__ out0, unsigned plane) {
   double a[6];
   hermite_coeff(M, u, A, a);
   const double U[3] = {u[0] + 0.5 * A[0], u[1] + 0.5 * A[1], u[2] + 0.5 * A[2]};
@@ -181,14 +183,14 @@ __device__ __forceinline__ void collide_store(const KP& P, const Moments& M, con
   T[5] = u[1] * u[2] + P.one_m_omega * a[5] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
   hermite2_populations(M.p, U, T, f);
 #pragma unroll
-  for (int i = 0; i < Q; ++i) Pop<ST>::store(fout + (size_t)i * P.G.n + k, i, f[i]);
+  for (int i = 0; i < Q; ++i) Pop<ST>::store(out0 + (unsigned)i * plane, i, f[i]);  // out0 = f*_0 of this node
 }
 
 template <typename ST>
 __device__ __forceinline__ void collide_store(const KP& P, const Moments& M, const double (&u)[3], const double (&A)[3],
-                                              ST* __restrict__ fout, unsigned k) {
+                                              ST* __restrict__ out0, unsigned plane) {
   double f[Q];
-  collide_store<ST>(P, M, u, A, f, fout, k);
+  collide_store<ST>(P, M, u, A, f, out0, plane);
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
@@ -235,7 +237,8 @@ __global__ void __launch_bounds__(128) k_lb(KP P, const ST* __restrict__ fin, ST
     uout[P.G.n + k] = u[1];
     uout[2u * P.G.n + k] = u[2];
   }
-  collide_store<ST>(P, M, u, A, f, fout, k);
+  const unsigned plane = (unsigned)P.G.nx * (unsigned)P.G.ny;
+  collide_store<ST>(P, M, u, A, f, pop_slab(fout, P.G, z) + (nb.yr[1] + (unsigned)x), plane);
 }
 
 // a8: conservative Allen-Cahn update (Eq. 3), forward Euler (R13):
@@ -325,7 +328,9 @@ __global__ void __launch_bounds__(128) k_init(KP P, const double* __restrict__ r
   hermite2_populations(M.p, U, T, f);
 #pragma unroll
   for (int i = 0; i < Q; ++i)
-    Pop<ST>::store(fout + (size_t)i * P.G.n + nb.at(-cz_of(i), -cy_of(i), -cx_of(i)), i, f[i]);
+    Pop<ST>::store(pop_slab(fout, P.G, nb.z[1 - cz_of(i)]) +
+                       ((unsigned)i * ((unsigned)P.G.nx * (unsigned)P.G.ny) + nb.yr[1 - cy_of(i)] + (unsigned)nb.x[1 - cx_of(i)]),
+                   i, f[i]);
 }
 
 // a9: (p*, u) of the current state; the state is unchanged.
@@ -494,6 +499,7 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
   if (!p) return false;
   if (nx < 4 || ny < 4 || nz < 4 || (nx & 1)) return false;
   if ((double)nx * (double)ny * (double)nz >= 2147483648.0) return false;
+  if (27.0 * (double)nx * (double)ny >= 4294967296.0) return false;  // 32-bit offsets inside a [27][ny][nx] slab
   if (!(p->tau > 0.5) || !std::isfinite(p->tau)) return false;
   if (p->force_type < 0 || p->force_type > 2) return false;
   if (p->two_phase) {

@@ -41,7 +41,7 @@ enum { ST_N = 0, ST_LB = 1, ST_K = 2, ST_ADV = 3 };
 
 struct PipeArgs {
   KP P;
-  const void* fin;    // populations of time t (post-collision, not yet streamed), [27][nz][ny][nx]
+  const void* fin;    // populations of time t (post-collision, not yet streamed), [nz][27][ny][nx]
   void* fout;         // populations of time t+1
   const double* phi;  // phi(t), [nz][ny][nx]
   double* phi_new;    // phi(t+1)
@@ -229,7 +229,7 @@ __device__ __forceinline__ void stage_LB(const PipeArgs& a, int zz, int item) {
   uo[0] = u[0];
   uo[plane] = u[1];
   uo[2 * plane] = u[2];
-  collide_store<ST>(P, M, u, A, f, (ST*)a.fout, k);
+  collide_store<ST>(P, M, u, A, f, pop_slab((ST*)a.fout, G, z) + idx, plane);
 }
 
 // ---------------------------------------------------------------------------------------------------- stage ADV

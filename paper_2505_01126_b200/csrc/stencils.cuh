@@ -19,7 +19,9 @@ struct Grid {
 // (compare-select, no modulo), replacing the paper's halo exchange.
 struct Nbr {
   int x[3];            // x-1, x, x+1 wrapped
-  unsigned row[3][3];  // [dz+1][dy+1] -> (zz * ny + yy) * nx
+  unsigned row[3][3];  // [dz+1][dy+1] -> (zz * ny + yy) * nx   (scalar fields, [z][y][x])
+  int z[3];            // z-1, z, z+1 wrapped                    (populations, [z][i][y][x])
+  unsigned yr[3];      // yy * nx
   __device__ __forceinline__ unsigned at(int dz, int dy, int dx) const { return row[dz + 1][dy + 1] + x[dx + 1]; }
 };
 
@@ -38,9 +40,24 @@ __device__ __forceinline__ void make_nbr(const Grid& G, int x, int y, int z, Nbr
   const int ys[3] = {wrap_dec(y, G.ny), y, wrap_inc(y, G.ny)};
   const int zs[3] = {wrap_dec(z, G.nz), z, wrap_inc(z, G.nz)};
 #pragma unroll
-  for (int a = 0; a < 3; ++a)
+  for (int a = 0; a < 3; ++a) {
+    nb.z[a] = zs[a];
+    nb.yr[a] = (unsigned)ys[a] * (unsigned)G.nx;
 #pragma unroll
     for (int b = 0; b < 3; ++b) nb.row[a][b] = ((unsigned)zs[a] * (unsigned)G.ny + (unsigned)ys[b]) * (unsigned)G.nx;
+  }
+}
+
+// Population storage: [z][i][y][x] -- for every z plane the 27 population planes lie next to each other.  The address of
+// f_i at (z, y, x) is base(z) + (i * plane + y * nx + x) with a 64-bit base per z plane and a 32-bit in-slab offset
+// (27 * nx * ny < 2^32 is checked at create), which costs two integer instructions per access instead of five for the
+// [i][z][y][x] layout (64-bit i * n + offset), and keeps the 27 + 27 streams of a step inside a few 2 MB pages per plane.
+template <typename T>
+__device__ __forceinline__ T* pop_slab(T* f, const Grid& G, int z) {
+  T* p = f + (size_t)z * 27u * ((size_t)G.nx * (size_t)G.ny);
+  asm("" : "+l"(p));  // keep the slab base a pointer in a register pair: the compiler otherwise folds it back into a
+                      // 64-bit index computation per access
+  return p;
 }
 
 // Lattice derivative along AX of a periodic field given through `val(dz, dy, dx)`.

@@ -120,11 +120,11 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
 
   // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1), as 27 asynchronous copies
   auto prefetch_pull = [&](int z) {
-    const unsigned zr[3] = {(unsigned)wrap_dec(z, G.nz) * plane, (unsigned)z * plane, (unsigned)wrap_inc(z, G.nz) * plane};
+    const ST* slab[3] = {pop_slab(fin, G, wrap_dec(z, G.nz)), pop_slab(fin, G, z), pop_slab(fin, G, wrap_inc(z, G.nz))};
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
-      const unsigned src = zr[1 - cz_of(i)] + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)];
-      cp_async_pop<(int)sizeof(ST)>(&S.fpop[i][tid], fin + (size_t)i * G.n + src);
+      const unsigned off = (unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)];
+      cp_async_pop<(int)sizeof(ST)>(&S.fpop[i][tid], slab[1 - cz_of(i)] + off);
     }
     cp_async_commit();
   };
@@ -285,7 +285,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       uout[k] = u[0];
       uout[G.n + k] = u[1];
       uout[2u * G.n + k] = u[2];
-      collide_store<ST>(P, M, u, A, fout, k);
+      collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + (yrow[1] + (unsigned)xs[1]), plane);
     }
     an0 = an1; an1 = an2; bn0 = bn1; bn1 = bn2;
     aq0 = aq1; aq1 = aq2; bq0 = bq1; bq1 = bq2;
