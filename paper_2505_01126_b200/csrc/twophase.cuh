@@ -164,22 +164,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   }
   __syncthreads();
 
+  int zq2 = pmod(z0 + 1, G.nz);  // wrapped zc + 2, carried (no integer division in the march)
   for (int zc = z0 - 1; zc <= z1; ++zc) {
     const int it = zc - (z0 - 1);  // 0, 1, 2, ...
-    // body-force density of the node updated in this iteration (plane zc-1), R20; loaded before the barriers
-    double Fb[3] = {0.0, 0.0, 0.0};
-    if (P.force_type != 0 && zc > z0 - 1) {
-      const double fsz = __ldg(tabs + 2 * (G.nx + G.ny) + (zc - 1)), fcz = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + (zc - 1));
-      if (P.force_type == 1) {  // ABC
-        Fb[0] = P.force_amp * (fsz + fcy);
-        Fb[1] = P.force_amp * (fsx + fcz);
-        Fb[2] = P.force_amp * (fsy + fcx);
-      } else {  // sine variant of BASELINE config 2
-        Fb[0] = P.force_amp * fsy;
-        Fb[1] = P.force_amp * fsz;
-        Fb[2] = P.force_amp * fsx;
-      }
-    }
     // ---- phi(zc+1) has landed (this thread's own elements); fetch phi(zc+2); z combinations of plane zc
     {
       cp_async_wait_but<1>();
@@ -188,11 +175,12 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const double* rp = &S.raw[(it + 2) & 3][0][0];  // plane zc+1
       double* rn = &S.raw[(it + 3) & 3][0][0];        // plane zc+2, last read (as plane zc-2) by this same thread
       if (zc < z1) {
-        const double* src = phi + (size_t)pmod(zc + 2, G.nz) * plane;
+        const double* src = phi + (size_t)zq2 * plane;
         cp_async_f64(rn + o2, src + o2off);
         if (r2 >= 0) cp_async_f64(rn + r2, src + r2off);
       }
       cp_async_commit();
+      zq2 = wrap_inc(zq2, G.nz);
       double* tz = &S.Tz[0][0];
       double* dz = &S.Dz[0][0];
       const double v = rp[o2], m = rm[o2];
@@ -279,6 +267,20 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const unsigned k = (unsigned)z * plane + yrow[1] + (unsigned)xs[1];
       rout[k] = P.D * lapp - P.kappa * divq;  // phi-only part of Eq. 3
 
+      // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
+      double Fb[3] = {0.0, 0.0, 0.0};
+      if (P.force_type != 0) {
+        const double fsz = __ldg(tabs + 2 * (G.nx + G.ny) + (zc - 1)), fcz = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + (zc - 1));
+        if (P.force_type == 1) {  // ABC
+          Fb[0] = P.force_amp * (fsz + fcy);
+          Fb[1] = P.force_amp * (fsx + fcz);
+          Fb[2] = P.force_amp * (fsy + fcx);
+        } else {  // sine variant of BASELINE config 2
+          Fb[0] = P.force_amp * fsy;
+          Fb[1] = P.force_amp * fsz;
+          Fb[2] = P.force_amp * fsx;
+        }
+      }
       double A[3], rho;
       accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, true, A, rho);
       const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
