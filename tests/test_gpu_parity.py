@@ -184,6 +184,31 @@ def test_two_phase_ragged_box_ratio10_with_forcing(acclb, shape):
     assert abs(dg["sum_phi"] - do["sum_phi"]) <= 1e-12 * do["sum_phi"]
 
 
+@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("shape", [(4, 4, 4), (6, 4, 8), (8, 12, 4)])
+def test_two_phase_minimum_size_boxes(acclb, shape, variant):
+    """The smallest boxes the ABI admits (nx, ny, nz >= 4): every tile wraps onto itself several times, the WENO5
+    stencil (radius 3) reaches round the periodic box, one z chunk holds the whole column.  Small-radius droplet,
+    density ratio 3, sine forcing; every kernel variant."""
+    nx, ny, nz = shape
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    md = lambda i, c, n: np.minimum(np.abs(i - c), n - np.abs(i - c))
+    r = np.sqrt(md(x, 1.0, nx) ** 2 + md(y, 1.5, ny) ** 2 + md(z, 0.5, nz) ** 2)
+    phi = 0.5 * (1.0 + np.tanh(2.0 * (1.6 - r) / 4.0))
+    X, Y, Z = 2 * np.pi * x / nx, 2 * np.pi * y / ny, 2 * np.pi * z / nz
+    u = np.stack([0.02 * np.sin(Y) * np.cos(Z), 0.015 * np.sin(Z + X), -0.01 * np.cos(X) * np.sin(Y)])
+    cfg = dict(n=None, rho=np.ones((nz, ny, nx)), u=np.ascontiguousarray(u), phi=np.ascontiguousarray(phi),
+               params=dict(tau=0.7, two_phase=1, rho_l=3.0, rho_g=1.0, sigma=0.005, mobility=0.05, width=4.0,
+                           force_type=2, force_amp=1e-5, force_k=1))
+    sim, o = gpu_sim(acclb, cfg, shape=shape), cpu_sim(cfg, shape=shape)
+    sim.set_variant(variant)
+    sim.step(8)
+    o.step(8)
+    assert_parity(sim, o)
+    dg, do = sim.diagnostics(), o.diagnostics()
+    assert abs(dg["sum_phi"] - do["sum_phi"]) <= 1e-12 * do["sum_phi"]
+
+
 def test_thin_slab_flat_interface(acclb):
     """Smallest legal box (4 x 4 x 64): every stencil wraps onto itself; flat interface pair (P9 set-up)."""
     nx, ny, nz = 4, 4, 64
