@@ -64,6 +64,8 @@ struct GeoTile {
   double Dz[PY][PX];      // Dz phi at plane zc
   double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
   ST fpop[Q][TX * TY];    // landing zone of the prefetched populations of the next plane: slot [i][tid] is thread tid's
+  double ftab[2][64];     // sin / cos force table entries of this block's planes (lz <= 64): the streaming pulls evict
+                          // everything from L1, so a per-plane __ldg of the table would wait for L2 every plane
 };
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
@@ -161,6 +163,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   if (P.force_type != 0) {
     fsx = __ldg(tabs + xw); fcx = __ldg(tabs + G.nx + xw);
     fsy = __ldg(tabs + 2 * G.nx + yw); fcy = __ldg(tabs + 2 * G.nx + G.ny + yw);
+    if (tid < z1 - z0) {
+      S.ftab[0][tid] = __ldg(tabs + 2 * (G.nx + G.ny) + z0 + tid);
+      S.ftab[1][tid] = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + z0 + tid);
+    }
   }
   __syncthreads();
 
@@ -270,7 +276,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
       double Fb[3] = {0.0, 0.0, 0.0};
       if (P.force_type != 0) {
-        const double fsz = __ldg(tabs + 2 * (G.nx + G.ny) + (zc - 1)), fcz = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + (zc - 1));
+        const double fsz = S.ftab[0][z - z0], fcz = S.ftab[1][z - z0];
         if (P.force_type == 1) {  // ABC
           Fb[0] = P.force_amp * (fsz + fcy);
           Fb[1] = P.force_amp * (fsx + fcz);
