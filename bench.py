@@ -289,11 +289,13 @@ def roofline_of(meas, steps, fp32):
          "step_bytes_per_lup": step_bytes_per_lup(fp32, meas["two_phase"])}
     r["step_achieved"] = r["step_bytes_per_lup"] * n3 * steps / (meas["ms"] * 1e-3) / 1e9
     r["step_frac"] = r["step_achieved"] / peak
-    t = ROOT / "profiles" / "traffic.json"  # dram bytes per launch of the kernel from the committed ncu --set full capture
+    t = ROOT / "profiles" / "r01_traffic.csv"  # dram bytes per launch of the kernel from the committed ncu --set full capture
     try:
-        tj = json.loads(t.read_text())
         key = f"{name}_{'two' if meas['two_phase'] else 'single'}_{'fp32' if fp32 else 'fp64'}_{meas['n']}"
-        r["traffic"] = tj.get(key)
+        for line in t.read_text().splitlines()[1:]:
+            k, v = line.split(",")
+            if k == key:
+                r["traffic"] = int(v)
     except Exception:
         pass
     return r
