@@ -60,8 +60,6 @@ struct GeoTile {
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
   double raw[4][PY][PX];  // ring of raw phi planes zc-1, zc, zc+1 and zc+2 (landing, cp.async)
-  double Tz[PY][PX];      // Sz phi at plane zc
-  double Dz[PY][PX];      // Dz phi at plane zc
   double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
   ST fpop[Q][TX * TY];    // landing zone of the prefetched populations of the next plane: slot [i][tid] is thread tid's
   double ftab[2][64];     // sin / cos force table entries of this block's planes (lz <= 64): the streaming pulls evict
@@ -69,9 +67,9 @@ struct GeoTile {
 };
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
-// Iteration zc: stage phi(zc+1) -> Sz, Dz of plane zc | derive n, q (tile + 1) and g, |g|, lap (own node, kept in
-// registers) on plane zc | plane sums of plane zc, then the node update of plane z = zc - 1, whose z combinations need
-// planes zc-2 .. zc (carried in registers).
+// Iteration zc: phi(zc+1) has landed, fetch phi(zc+2) | derive n, q (tile + 1) and g, |g|, lap (own node, kept in
+// registers) on plane zc from the raw planes zc-1, zc, zc+1 | plane sums of plane zc, then the node update of plane
+// z = zc - 1, whose z combinations need planes zc-2 .. zc (carried in registers).
 // The 27 populations a thread pulls for plane z are fetched with cp.async into the thread's own shared-memory slots while
 // the block is still busy with plane z-1 and with the geometry of plane z: the HBM latency of the pull hides under the
 // fp64 work instead of stalling every warp at the top of the node update, and no register holds a load in flight.
@@ -173,13 +171,11 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   int zq2 = pmod(z0 + 1, G.nz);  // wrapped zc + 2, carried (no integer division in the march)
   for (int zc = z0 - 1; zc <= z1; ++zc) {
     const int it = zc - (z0 - 1);  // 0, 1, 2, ...
-    // ---- phi(zc+1) has landed (this thread's own elements); fetch phi(zc+2); z combinations of plane zc
+    // ---- phi(zc+1) has landed (this thread's own elements); fetch phi(zc+2)
     {
       cp_async_wait_but<1>();
-      const double* rm = &S.raw[it & 3][0][0];        // plane zc-1
-      const double* rc = &S.raw[(it + 1) & 3][0][0];  // plane zc
-      const double* rp = &S.raw[(it + 2) & 3][0][0];  // plane zc+1
-      double* rn = &S.raw[(it + 3) & 3][0][0];        // plane zc+2, last read (as plane zc-2) by this same thread
+      double* rn = &S.raw[(it + 3) & 3][0][0];        // plane zc+2: its slot held plane zc-2, last read before the
+                                                      // previous iteration's second barrier
       if (zc < z1) {
         const double* src = phi + (size_t)zq2 * plane;
         cp_async_f64(rn + o2, src + o2off);
@@ -187,37 +183,38 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       }
       cp_async_commit();
       zq2 = wrap_inc(zq2, G.nz);
-      double* tz = &S.Tz[0][0];
-      double* dz = &S.Dz[0][0];
-      const double v = rp[o2], m = rm[o2];
-      tz[o2] = fma(4.0, rc[o2], m + v);
-      dz[o2] = v - m;
-      if (r2 >= 0) {
-        const double v2 = rp[r2], m2 = rm[r2];
-        tz[r2] = fma(4.0, rc[r2], m2 + v2);
-        dz[r2] = v2 - m2;
-      }
     }
     __syncthreads();
     // ---- derive n, q (tile + 1 rim) and g, |g|, lap (own node) on plane zc           PAPER.md:L61, L104; R17
     double gc[3], gnc, lapc;
     {
-      const double* rc = &S.raw[(it + 1) & 3][0][0];
+      const double* rm = &S.raw[it & 3][0][0];        // plane zc-1
+      const double* rc = &S.raw[(it + 1) & 3][0][0];  // plane zc
+      const double* rp = &S.raw[(it + 2) & 3][0][0];  // plane zc+1
       auto derive = [&](int j, int i, bool own_node) {  // (j, i) in the NY x NX plane; centre (j+1, i+1) in a phi plane
-        const double* t = &S.Tz[j][i];
-        const double* d = &S.Dz[j][i];
         constexpr int PX = T::PX;
-        const double t00 = t[0], t01 = t[1], t02 = t[2], t10 = t[PX], t11 = t[PX + 1], t12 = t[PX + 2];
-        const double t20 = t[2 * PX], t21 = t[2 * PX + 1], t22 = t[2 * PX + 2];
+        const int b = j * PX + i;
+        // z combinations of the nine columns around the node: t = Sz phi = (1,4,1).phi, d = Dz phi = phi(z+1) - phi(z-1)
+        double t[9], d[9], ph = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            const int e = b + a * PX + c;
+            const double m = rm[e], v = rc[e], p = rp[e];
+            t[3 * a + c] = fma(4.0, v, m + p);
+            d[3 * a + c] = p - m;
+            if (a == 1 && c == 1) ph = v;
+          }
+        const double t00 = t[0], t01 = t[1], t02 = t[2], t10 = t[3], t11 = t[4], t12 = t[5], t20 = t[6], t21 = t[7], t22 = t[8];
         const double gx = (1.0 / 72.0) * fma(4.0, t12 - t10, (t02 - t00) + (t22 - t20));
         const double gy = (1.0 / 72.0) * fma(4.0, t21 - t01, (t20 - t00) + (t22 - t02));
         const double r0 = fma(4.0, d[1], d[0] + d[2]);
-        const double r1 = fma(4.0, d[PX + 1], d[PX] + d[PX + 2]);
-        const double r2_ = fma(4.0, d[2 * PX + 1], d[2 * PX] + d[2 * PX + 2]);
+        const double r1 = fma(4.0, d[4], d[3] + d[5]);
+        const double r2_ = fma(4.0, d[7], d[6] + d[8]);
         const double gz = (1.0 / 72.0) * fma(4.0, r1, r0 + r2_);
         const double gn = sqrt(fma(gx, gx, fma(gy, gy, gz * gz)));
         const double inv = div_pos(1.0, gn + 1e-12);
-        const double ph = rc[(j + 1) * PX + (i + 1)];
         const double pq = ph * (1.0 - ph);
         const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
         S.nq[0][j][i] = nx_;
