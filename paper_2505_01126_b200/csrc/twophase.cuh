@@ -42,6 +42,30 @@ __device__ __forceinline__ void cp_async_pop(void* smem, const void* gmem) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(sa), "l"(gmem), "n"(BYTES) : "memory");
 }
+// mbarrier + TMA (tiled bulk tensor copy) primitives for the population pull of interior tiles.
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+  asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(b);
+  unsigned done;
+  do {
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done) : "r"(a), "r"(parity) : "memory");
+  } while (!done);
+}
+// One TX x TY x 1 box of a rank-3 tensor (x, y, slab = z * 27 + i) -> shared memory, completion in bytes on the mbarrier.
+__device__ __forceinline__ void tma_load_box(void* smem, const void* tmap, int cx, int cy, int cs, unsigned long long* b) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(smem)),
+               "l"(tmap), "r"(cx), "r"(cy), "r"(cs), "r"((unsigned)__cvta_generic_to_shared(b))
+               : "memory");
+}
+
 __device__ __forceinline__ void cp_async_f64(double* smem, const double* gmem) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
@@ -51,17 +75,37 @@ __device__ __forceinline__ void cp_async_wait_but() { asm volatile("cp.async.wai
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+// Landing zone of the pull: population i occupies a dense TY x W_i box, W_i = TX for c_ix = 0 and TX + 2 otherwise.  TMA
+// needs a 16-byte aligned box start, i.e. an even x for fp64, so the x-shifted populations are fetched as the aligned window
+// x0 - 2 .. x0 + TX - 1 (c_ix = +1) or x0 .. x0 + TX + 1 (c_ix = -1) -- the two extra elements lie in 32-byte sectors the
+// pull touches anyway -- and thread tx reads element tx + 1 of its row.
+template <int TX>
+__host__ __device__ constexpr int pull_w(int i) { return cx_of(i) == 0 ? TX : TX + 2; }
+template <int TX, int TY>
+__host__ __device__ constexpr int pull_off(int i) {
+  int o = 0;
+  for (int j = 0; j < i; ++j) o += TY * pull_w<TX>(j);
+  return o;
+}
+template <int TX, int TY>
+__host__ __device__ constexpr int pull_slot(int i, int tx, int ty) {
+  return pull_off<TX, TY>(i) + ty * pull_w<TX>(i) + tx + (cx_of(i) == 0 ? 0 : 1);
+}
+
 // Shared-memory working set of k_lb_tp for one TX x TY column marching along z.
 //   The D3Q27 stencil weights factorise, w_i = W(cx) W(cy) W(cz) / 216 with W = (1,4,1), so every lattice stencil of
 //   PAPER.md:L104 is evaluated separably: a z combination per (x,y) column first (Sz = (1,4,1), Dz = (+1,0,-1)), then a
 //   3 x 3 stencil in the plane.  Same numbers as the 27-term sums up to rounding order.
 template <typename ST, int TX, int TY>
 struct GeoTile {
+  // landing zone of the pulled populations of the next plane (layout: pull_slot above); for interior tiles the TMA writes
+  // population i's box here in one piece (128-byte aligned destinations: TY * W_i * 8 is a multiple of 128)
+  alignas(128) ST fpop[pull_off<TX, TY>(Q)];
+  unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
   double raw[4][PY][PX];  // ring of raw phi planes zc-1, zc, zc+1 and zc+2 (landing, cp.async)
   double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
-  ST fpop[Q][TX * TY];    // landing zone of the prefetched populations of the next plane: slot [i][tid] is thread tid's
   double ftab[2][64];     // sin / cos force table entries of this block's planes (lz <= 64): the streaming pulls evict
                           // everything from L1, so a per-plane __ldg of the table would wait for L2 every plane
 };
@@ -76,9 +120,10 @@ struct GeoTile {
 template <typename ST, int TX, int TY, int MINB>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
-        double* __restrict__ uout, double* __restrict__ rout, const double* __restrict__ tabs, int lz) {
+        double* __restrict__ uout, double* __restrict__ rout, const double* __restrict__ tabs, int lz,
+        const __grid_constant__ CUtensorMap tmap_fin, const __grid_constant__ CUtensorMap tmap_fin_wide, int use_tma) {
   using T = GeoTile<ST, TX, TY>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   T& S = *reinterpret_cast<T*>(smem_raw);
   constexpr int NT = TX * TY;
   constexpr int RIM2 = T::PX * T::PY - NT;  // staging items besides the thread's own node
@@ -119,12 +164,38 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
                             (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx};
 
   // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1), as 27 asynchronous copies
+  // Interior tiles (no periodic wrap in x or y inside the shifted boxes): ONE thread issues 27 tiled TMA loads, population i's
+  // TX x TY box shifted by -c_i straight into fpop[i]; completion is counted in bytes on an mbarrier.  No per-thread copy
+  // instructions, no address registers held by copies in flight, no L1 allocation.  Tiles on the x / y rim of the box (TMA
+  // zero-fills out of bounds, it does not wrap) and tensors the map cannot describe use the per-thread cp.async pull.
+  const bool fast = use_tma && x0 >= 2 && x0 + TX + 2 <= G.nx && y0 >= 1 && y0 + TY + 1 <= G.ny;  // block-uniform
+  auto tma_pull = [&](int z) {  // called by thread 0 only
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_arrive_expect_tx(&S.fbar, (unsigned)(pull_off<TX, TY>(Q) * sizeof(ST)));
+    const int zs[3] = {wrap_dec(z, G.nz) * Q, z * Q, wrap_inc(z, G.nz) * Q};
+#pragma unroll
+    for (int i = 0; i < Q; ++i)
+      tma_load_box(&S.fpop[pull_off<TX, TY>(i)], cx_of(i) == 0 ? (const void*)&tmap_fin : (const void*)&tmap_fin_wide,
+                   cx_of(i) == 1 ? x0 - 2 : x0, y0 - cy_of(i), zs[1 - cz_of(i)] + i, &S.fbar);
+  };
+  if (fast) {
+    if (tid == 0) {
+      mbar_init(&S.fbar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) tma_pull(z0);
+  }
   auto prefetch_pull = [&](int z) {
+    if (fast) {  // the TMA pull is issued by thread 0 after the block-wide hand-over below
+      cp_async_commit();
+      return;
+    }
     const ST* slab[3] = {pop_slab(fin, G, wrap_dec(z, G.nz)), pop_slab(fin, G, z), pop_slab(fin, G, wrap_inc(z, G.nz))};
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
       const unsigned off = (unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)];
-      cp_async_pop<(int)sizeof(ST)>(&S.fpop[i][tid], slab[1 - cz_of(i)] + off);
+      cp_async_pop<(int)sizeof(ST)>(&S.fpop[pull_slot<TX, TY>(i, tx, ty)], slab[1 - cz_of(i)] + off);
     }
     cp_async_commit();
   };
@@ -257,9 +328,14 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     if (!(z >= z0 && active)) cp_async_commit();
     if (z >= z0 && active) {
       // a1-a2: the pulled populations have landed in this thread's slots; moments, then refill the slots for plane z+1
-      cp_async_wait_but<1>();
+      if (fast) mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
+      else cp_async_wait_but<1>();
       Moments M;
-      moments_of([&](int i) { return Pop<ST>::from_storage(S.fpop[i][tid], i); }, M);
+      moments_of([&](int i) { return Pop<ST>::from_storage(S.fpop[pull_slot<TX, TY>(i, tx, ty)], i); }, M);
+      if (fast) {  // every warp has read its 27 values out of the landing zone: refill it for plane z+1
+        __syncthreads();
+        if (tid == 0 && z + 1 < z1) tma_pull(z + 1);
+      }
       if (z + 1 < z1) prefetch_pull(z + 1);
       else cp_async_commit();
       // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
