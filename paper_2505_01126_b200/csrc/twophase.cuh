@@ -123,8 +123,8 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         double* __restrict__ uout, double* __restrict__ rout, const double* __restrict__ tabs, int lz,
         const __grid_constant__ CUtensorMap tmap_fin, const __grid_constant__ CUtensorMap tmap_fin_wide, int use_tma) {
   using T = GeoTile<ST, TX, TY>;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  T& S = *reinterpret_cast<T*>(smem_raw);
+  extern __shared__ __align__(128) unsigned char smem_lb[];
+  T& S = *reinterpret_cast<T*>(smem_lb);
   constexpr int NT = TX * TY;
   constexpr int RIM2 = T::PX * T::PY - NT;  // staging items besides the thread's own node
   constexpr int RIM1 = T::NX * T::NY - NT;  // derive items besides the thread's own node
@@ -394,8 +394,8 @@ __global__ void __launch_bounds__(TX * TY, 4)
 k_advect(KP P, const double* __restrict__ phi, const double* __restrict__ u, const double* __restrict__ r,
          double* __restrict__ phi_new, int lz) {
   using T = AdvTile<TX, TY>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T& S = *reinterpret_cast<T*>(smem_raw);
+  extern __shared__ __align__(128) unsigned char smem_lb[];
+  T& S = *reinterpret_cast<T*>(smem_lb);
   constexpr int NT = TX * TY;
   static_assert(TX == 32 && TY >= 8 && 6 * (TX + TY) <= NT && 2 * (TX + TY) <= NT, "one warp per tile row, one halo element per thread");
   const Grid& G = P.G;
