@@ -449,7 +449,7 @@ struct accLB_ctx {
   double* nrm;
   double* tabs;
   double* acc;
-  CUtensorMap tmap[2][2];  // populations A / B as rank-3 tensors (x, y, z * 27 + i), box width TX | TX + 2, for the TMA pull
+  CUtensorMap tmap[2];  // populations A / B as rank-3 tensors (x, y, z * 27 + i) for the TMA pull of k_lb_tp
   int tmap_ok;          // 0: tensor maps unavailable (shape the map cannot describe, or no driver entry point)
   double* rings;  // pipeline ring buffers: n(3) | g,c(4) | r | u(3) | fz, a few planes each (two-phase)
   int* sync;      // pipeline counters: ticket | done[4][nz + 4]
@@ -568,7 +568,7 @@ static int launch_lb_tp(accLB_ctx* s, int c, int d) {
   const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
   LaunchScope ls(s, KIND_LB);
   kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], s->u, s->r,
-                                                        s->tabs, lz, s->tmap[c][0], s->tmap[c][1], s->tmap_ok);
+                                                        s->tabs, lz, s->tmap[c], s->tmap_ok);
   return ACCLB_OK;
 }
 
@@ -632,7 +632,7 @@ static int launch_step_tp(accLB_ctx* s, int c, int d) {
 }
 
 // Tensor maps of the two population buffers for the tiled TMA pull (k_lb_tp): rank 3, (x, y, slab = z * 27 + i), box
-// LBT_TX (or LBT_TX + 2, for the x-shifted populations) x LBT_TY x 1, no swizzle, zero fill out of bounds.  Returns 1 on success; 0 (the kernels then use the per-thread
+// LBT_TX x LBT_TY x 1 (unshifted in x: box starts must be 16-byte aligned), no swizzle, zero fill out of bounds.  Returns 1 on success; 0 (the kernels then use the per-thread
 // cp.async pull everywhere) when the driver entry point is missing or the shape violates a tensor-map constraint.
 static int make_tensor_maps(accLB_ctx* s) {
   typedef CUresult (*encode_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -645,20 +645,18 @@ static int make_tensor_maps(accLB_ctx* s) {
     cudaGetLastError();
     return 0;
   }
-  if (s->prm.store_fp32) return 0;  // 16-byte aligned box starts would need 4-element windows: fp32 storage keeps cp.async
-  const size_t es = 8;
-  if (((size_t)s->nx * es) % 16 != 0 || s->nx < LBT_TX + 2 || s->ny < LBT_TY) return 0;
+  const size_t es = s->prm.store_fp32 ? 4 : 8;
+  if (((size_t)s->nx * es) % 16 != 0 || s->nx < LBT_TX || s->ny < LBT_TY) return 0;
   const cuuint64_t dims[3] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny, (cuuint64_t)27 * s->nz};
   const cuuint64_t strides[2] = {(cuuint64_t)s->nx * es, (cuuint64_t)s->nx * s->ny * es};
-  const cuuint32_t estr[3] = {1, 1, 1};
-  for (int b = 0; b < 2; ++b)
-    for (int w = 0; w < 2; ++w) {
-      const cuuint32_t box[3] = {(cuuint32_t)(LBT_TX + 2 * w), LBT_TY, 1};
-      const CUresult r = ((encode_t)fn)(&s->tmap[b][w], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, s->f[b], dims, strides, box, estr,
-                                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                        CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) return 0;
-    }
+  const cuuint32_t box[3] = {LBT_TX, LBT_TY, 1}, estr[3] = {1, 1, 1};
+  for (int b = 0; b < 2; ++b) {
+    const CUresult r = ((encode_t)fn)(&s->tmap[b], s->prm.store_fp32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
+                                      3, s->f[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return 0;
+  }
   return 1;
 }
 

@@ -75,32 +75,20 @@ __device__ __forceinline__ void cp_async_wait_but() { asm volatile("cp.async.wai
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// Landing zone of the pull: population i occupies a dense TY x W_i box, W_i = TX for c_ix = 0 and TX + 2 otherwise.  TMA
-// needs a 16-byte aligned box start, i.e. an even x for fp64, so the x-shifted populations are fetched as the aligned window
-// x0 - 2 .. x0 + TX - 1 (c_ix = +1) or x0 .. x0 + TX + 1 (c_ix = -1) -- the two extra elements lie in 32-byte sectors the
-// pull touches anyway -- and thread tx reads element tx + 1 of its row.
-template <int TX>
-__host__ __device__ constexpr int pull_w(int i) { return cx_of(i) == 0 ? TX : TX + 2; }
-template <int TX, int TY>
-__host__ __device__ constexpr int pull_off(int i) {
-  int o = 0;
-  for (int j = 0; j < i; ++j) o += TY * pull_w<TX>(j);
-  return o;
-}
-template <int TX, int TY>
-__host__ __device__ constexpr int pull_slot(int i, int tx, int ty) {
-  return pull_off<TX, TY>(i) + ty * pull_w<TX>(i) + tx + (cx_of(i) == 0 ? 0 : 1);
-}
-
 // Shared-memory working set of k_lb_tp for one TX x TY column marching along z.
 //   The D3Q27 stencil weights factorise, w_i = W(cx) W(cy) W(cz) / 216 with W = (1,4,1), so every lattice stencil of
 //   PAPER.md:L104 is evaluated separably: a z combination per (x,y) column first (Sz = (1,4,1), Dz = (+1,0,-1)), then a
 //   3 x 3 stencil in the plane.  Same numbers as the 27-term sums up to rounding order.
 template <typename ST, int TX, int TY>
 struct GeoTile {
-  // landing zone of the pulled populations of the next plane (layout: pull_slot above); for interior tiles the TMA writes
-  // population i's box here in one piece (128-byte aligned destinations: TY * W_i * 8 is a multiple of 128)
-  alignas(128) ST fpop[pull_off<TX, TY>(Q)];
+  // Landing zone of the pulled populations of the next plane.  For interior tiles the TMA writes population i's TX x TY box
+  // of rows y0 - c_iy, plane z - c_iz, UNSHIFTED in x (TMA needs 16-byte aligned box starts, and a window widened to the next
+  // aligned element costs a 64-byte DRAM fetch per row: measured +4.8 GB per 512^3 step), so thread tx reads element
+  // tx - c_ix of its row; the one element per row that lies outside the box (x0 - 1 for c_ix = +1, x0 + TX for c_ix = -1)
+  // is fetched by the edge lane itself with an 8-byte cp.async into the tail of the slab.
+  // One slab per population: the box, then the TY edge elements, padded to a multiple of 128 bytes (TMA destination).
+  static constexpr int SLAB = TX * TY + 128 / (int)sizeof(ST);
+  alignas(128) ST fpop[Q][SLAB];
   unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
@@ -121,7 +109,7 @@ template <typename ST, int TX, int TY, int MINB>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
         double* __restrict__ uout, double* __restrict__ rout, const double* __restrict__ tabs, int lz,
-        const __grid_constant__ CUtensorMap tmap_fin, const __grid_constant__ CUtensorMap tmap_fin_wide, int use_tma) {
+        const __grid_constant__ CUtensorMap tmap_fin, int use_tma) {
   using T = GeoTile<ST, TX, TY>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
@@ -163,20 +151,24 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const unsigned yrow[3] = {(unsigned)wrap_dec(yw, G.ny) * (unsigned)G.nx, (unsigned)yw * (unsigned)G.nx,
                             (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx};
 
-  // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1), as 27 asynchronous copies
-  // Interior tiles (no periodic wrap in x or y inside the shifted boxes): ONE thread issues 27 tiled TMA loads, population i's
-  // TX x TY box shifted by -c_i straight into fpop[i]; completion is counted in bytes on an mbarrier.  No per-thread copy
-  // instructions, no address registers held by copies in flight, no L1 allocation.  Tiles on the x / y rim of the box (TMA
-  // zero-fills out of bounds, it does not wrap) and tensors the map cannot describe use the per-thread cp.async pull.
-  const bool fast = use_tma && x0 >= 2 && x0 + TX + 2 <= G.nx && y0 >= 1 && y0 + TY + 1 <= G.ny;  // block-uniform
+  // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1).
+  // Tiles whose shifted rows stay inside the box in y (no periodic wrap: TMA zero-fills out of bounds) and that are full
+  // width: ONE thread issues 27 tiled TMA loads (cp.async.bulk.tensor), completion counted in bytes on an mbarrier; no
+  // per-thread copy instructions, no address registers held by copies in flight, no L1 allocation.  The two edge lanes of
+  // a row fetch the 9 + 9 elements outside the boxes themselves.  All other tiles: one 8-byte cp.async per thread and
+  // population.  Either way population i of thread (tx, ty) ends up at *slot(i).
+  const bool fast = use_tma && x0 + TX <= G.nx && y0 >= 1 && y0 + TY + 1 <= G.ny;  // block-uniform
+  // three per-thread bases, one per c_ix, so that slot(i) is base + a compile-time offset
+  ST* const sl_c = &S.fpop[0][ty * TX + tx];
+  ST* const sl_p = tx == 0 ? &S.fpop[0][NT + ty] : sl_c - 1;       // c_ix = +1: element x - 1
+  ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + ty] : sl_c + 1;  // c_ix = -1: element x + 1
+  auto slot = [&](int i) -> ST* { return (cx_of(i) == 0 ? sl_c : cx_of(i) == 1 ? sl_p : sl_m) + i * T::SLAB; };
   auto tma_pull = [&](int z) {  // called by thread 0 only
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    mbar_arrive_expect_tx(&S.fbar, (unsigned)(pull_off<TX, TY>(Q) * sizeof(ST)));
+    mbar_arrive_expect_tx(&S.fbar, (unsigned)(Q * NT * sizeof(ST)));
     const int zs[3] = {wrap_dec(z, G.nz) * Q, z * Q, wrap_inc(z, G.nz) * Q};
 #pragma unroll
-    for (int i = 0; i < Q; ++i)
-      tma_load_box(&S.fpop[pull_off<TX, TY>(i)], cx_of(i) == 0 ? (const void*)&tmap_fin : (const void*)&tmap_fin_wide,
-                   cx_of(i) == 1 ? x0 - 2 : x0, y0 - cy_of(i), zs[1 - cz_of(i)] + i, &S.fbar);
+    for (int i = 0; i < Q; ++i) tma_load_box(&S.fpop[i][0], &tmap_fin, x0, y0 - cy_of(i), zs[1 - cz_of(i)] + i, &S.fbar);
   };
   if (fast) {
     if (tid == 0) {
@@ -187,15 +179,16 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     if (tid == 0) tma_pull(z0);
   }
   auto prefetch_pull = [&](int z) {
-    if (fast) {  // the TMA pull is issued by thread 0 after the block-wide hand-over below
+    if (fast && tx != 0 && tx != TX - 1) {  // the boxes are on their way (thread 0, after the block-wide hand-over)
       cp_async_commit();
       return;
     }
     const ST* slab[3] = {pop_slab(fin, G, wrap_dec(z, G.nz)), pop_slab(fin, G, z), pop_slab(fin, G, wrap_inc(z, G.nz))};
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
+      if (fast && !((cx_of(i) == 1 && tx == 0) || (cx_of(i) == -1 && tx == TX - 1))) continue;
       const unsigned off = (unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)];
-      cp_async_pop<(int)sizeof(ST)>(&S.fpop[pull_slot<TX, TY>(i, tx, ty)], slab[1 - cz_of(i)] + off);
+      cp_async_pop<(int)sizeof(ST)>(slot(i), slab[1 - cz_of(i)] + off);
     }
     cp_async_commit();
   };
@@ -328,10 +321,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     if (!(z >= z0 && active)) cp_async_commit();
     if (z >= z0 && active) {
       // a1-a2: the pulled populations have landed in this thread's slots; moments, then refill the slots for plane z+1
+      cp_async_wait_but<1>();
       if (fast) mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
-      else cp_async_wait_but<1>();
       Moments M;
-      moments_of([&](int i) { return Pop<ST>::from_storage(S.fpop[pull_slot<TX, TY>(i, tx, ty)], i); }, M);
+      moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
       if (fast) {  // every warp has read its 27 values out of the landing zone: refill it for plane z+1
         __syncthreads();
         if (tid == 0 && z + 1 < z1) tma_pull(z + 1);
