@@ -96,6 +96,7 @@ struct GeoTile {
   double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
   double ftab[2][64];     // sin / cos force table entries of this block's planes (lz <= 64): the streaming pulls evict
                           // everything from L1, so a per-plane __ldg of the table would wait for L2 every plane
+  double ftx[2][TX], fty[2][TY];  // the same for the tile's columns and rows (kept here rather than in 8 registers)
 };
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
@@ -139,11 +140,13 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const int o2 = (ty + 2) * T::PX + (tx + 2);
   const unsigned o2off = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
   // rim item of the derive pass: element (j, i) of the NY x NX plane that is not an own node
-  int r1j = -1, r1i = 0;
+  int r1 = -1;  // j * NX + i (one register; j, i are recovered by a constant division where they are needed)
   if (tid < RIM1) {
+    int r1j, r1i;
     if (tid < T::NX) { r1j = 0; r1i = tid; }
     else if (tid < 2 * T::NX) { r1j = T::NY - 1; r1i = tid - T::NX; }
     else { const int e = tid - 2 * T::NX; r1j = 1 + (e >> 1); r1i = (e & 1) ? T::NX - 1 : 0; }
+    r1 = r1j * T::NX + r1i;
   }
 
   const int xw = pmod(x, G.nx), yw = pmod(y, G.ny);
@@ -220,11 +223,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   double an0 = 0.0, an1 = 0.0, bn0 = 0.0, bn1 = 0.0;  // plane sums of n at planes zc-2, zc-1
   double aq0 = 0.0, aq1 = 0.0, bq0 = 0.0, bq1 = 0.0;  // plane sums of q
   double gp[3] = {0.0, 0.0, 0.0}, gnp = 0.0, lapp = 0.0;  // g, |g|, lap phi of the own node at plane zc-1
-  // x- and y-dependent parts of the body force are fixed along the march (R20)
-  double fsx = 0.0, fcx = 0.0, fsy = 0.0, fcy = 0.0;
+  // x-, y- and z-dependent table entries of the body force (R20) of this tile and chunk
   if (P.force_type != 0) {
-    fsx = __ldg(tabs + xw); fcx = __ldg(tabs + G.nx + xw);
-    fsy = __ldg(tabs + 2 * G.nx + yw); fcy = __ldg(tabs + 2 * G.nx + G.ny + yw);
+    if (ty == 0) { S.ftx[0][tx] = __ldg(tabs + xw); S.ftx[1][tx] = __ldg(tabs + G.nx + xw); }
+    if (tx == 0) { S.fty[0][ty] = __ldg(tabs + 2 * G.nx + yw); S.fty[1][ty] = __ldg(tabs + 2 * G.nx + G.ny + yw); }
     if (tid < z1 - z0) {
       S.ftab[0][tid] = __ldg(tabs + 2 * (G.nx + G.ny) + z0 + tid);
       S.ftab[1][tid] = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + z0 + tid);
@@ -295,7 +297,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         }
       };
       derive(ty + 1, tx + 1, true);
-      if (r1j >= 0) derive(r1j, r1i, false);
+      if (r1 >= 0) derive(r1 / T::NX, r1 % T::NX, false);
     }
     __syncthreads();
     // ---- plane sums of plane zc at the own node:  a = Dx Sy v_x + Sx Dy v_y,  b = Sx Sy v_z
@@ -343,6 +345,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       double Fb[3] = {0.0, 0.0, 0.0};
       if (P.force_type != 0) {
         const double fsz = S.ftab[0][z - z0], fcz = S.ftab[1][z - z0];
+        const double fsx = S.ftx[0][tx], fcx = S.ftx[1][tx], fsy = S.fty[0][ty], fcy = S.fty[1][ty];
         if (P.force_type == 1) {  // ABC
           Fb[0] = P.force_amp * (fsz + fcy);
           Fb[1] = P.force_amp * (fsx + fcz);
