@@ -7,6 +7,9 @@
 //                                                                                     PAPER.md:L75-92 (Eqs. 4-7)
 //   k_allen_cahn (two-phase) conservative Allen-Cahn, flux-form WENO5 + lattice stencils, forward Euler (a8)
 //                                                                                     PAPER.md:L61-67 (Eq. 3)
+// These three are the one-node-per-thread kernels (single-phase default; two-phase variant 1).  The default two-phase
+// step is k_lb_tp + k_advect (twophase.cuh: shared-memory tiles marching along z, TMA / cp.async staging); variant 2 is
+// the persistent L2-pipeline kernel k_step_tp (pipeline.cuh).
 // State: post-collision, not yet streamed populations f*_i(x) in SoA [z][i][y][x], double-buffered (A/B), so the
 // pull f_i(x,t) = f*_i(x - c_i, t-1) reads shifted rows and every store is aligned; phi double-buffered.
 // No CPU fallback, no library kernels: everything the path computes runs in the kernels of this file.

@@ -11,6 +11,9 @@
 //               flux form (R12).  Every face flux is computed once per face (shared memory for x / y
 //               faces, a register carried along the z march for z faces), so sum phi is conserved to rounding.
 // Periodic boundaries are index wraps when the tiles are filled (PAPER.md:L114's halo exchange is not needed).
+// Staging: the 27 pulled populations of the next plane arrive by TMA (27 tiled cp.async.bulk.tensor box loads issued by
+// one thread, mbarrier completion) in tiles away from the y rim, by one cp.async per thread and population elsewhere; phi,
+// u, r planes arrive by cp.async one plane ahead.
 #pragma once
 
 namespace acclb {
