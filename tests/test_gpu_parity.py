@@ -352,7 +352,8 @@ def test_config4_full_size_512_sampled_against_oracle(acclb):
     variant, default stream): after k steps every node of three 44^3 sub-boxes (one wrapping the periodic corner, two
     cutting through bubble interfaces) is compared with the oracle run on that periodic sub-box, whose interior is
     exact beyond a rim of 3k + 2 nodes (tests/test_oracle_physics.py::test_subbox_evaluation_matches_full_box_interior).
-    Plus the properties that hold at any size: sum p* and sum phi conserved."""
+    Plus the properties that hold at any size, over the config's full 2000 steps: sum p* and sum phi conserved to 1e-12,
+    kinetic energy finite and of the initial order, |u| < 0.3."""
     free, _ = torch.cuda.mem_get_info()
     if free < 90e9:
         pytest.skip("needs about 80 GB of free device memory")
@@ -385,6 +386,14 @@ def test_config4_full_size_512_sampled_against_oracle(acclb):
         pin = po[inner]
         seen_interface |= bool(((pin > 0.1) & (pin < 0.9)).any())
     assert seen_interface, "no sampled box cut through an interface"
+    # ... and on to the full length of the config (2000 steps, diagnostics every 500): the invariants that hold at any size
+    for _ in range(4):
+        sim.step(500 if _ else 500 - k)
+        d = sim.diagnostics()
+        assert abs(d["sum_phi"] - d0["sum_phi"]) <= 1e-12 * d0["sum_phi"], d
+        assert abs(d["sum_pstar"] - d0["sum_pstar"]) <= 1e-12 * n ** 3, d
+        assert np.isfinite(d["ke"]) and 0.2 * d0["ke"] < d["ke"] < 2.0 * d0["ke"] and d["umax"] < 0.3, d
+    assert d["step"] == 2000
 
 
 # ---------------------------------------------------------------------------------------------- config 3 at full size
