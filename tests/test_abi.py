@@ -61,6 +61,7 @@ def test_workspace_bytes(lib):
     ((32, 32, 32), dict(tau=0.8, two_phase=1, width=0.0)),
     ((32, 32, 32), dict(tau=0.8, two_phase=1, rho_g=0.0)),
     ((2048, 2048, 1024), dict(tau=0.8)),      # >= 2^31 nodes
+    ((16384, 16384, 4), dict(tau=0.8)),       # 27 nx ny >= 2^32: in-slab offsets of the [z][i][y][x] layout are 32-bit
 ])
 def test_invalid_arguments_give_zero_workspace(lib, shape, kw):
     assert binding.workspace_bytes(*shape, binding.make_params(**kw)) == 0
