@@ -17,8 +17,9 @@
  * (x+c+N)%N periodic wraps.  Build with -ffp-contract=off so the arithmetic is what is written.
  *
  * Parity-unpinned parts (the paper fixes nothing to pin them against):
- *   - WENO5 variant / epsilon (R12), forward-Euler phi integrator (R13), step ordering (R14),
- *     index contraction of the viscous-correction force F^nu (R9).
+ *   - WENO5 variant / epsilon (R12), forward-Euler phi integrator (R13), step ordering (R14).
+ *   Pinned since round 2 (tests/test_oracle_physics.py): direction, upwind side and order of the phi advection
+ *   (face_flux / pass_allen_cahn), and F^nu (R9) on a prescribed shear against nu (du + du^T).grad rho.
  */
 #include <math.h>
 #include <stdlib.h>

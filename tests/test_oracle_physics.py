@@ -348,3 +348,162 @@ def test_subbox_evaluation_matches_full_box_interior():
     inner = (slice(rim, s - rim),) * 3
     for a, b in zip(full, got):
         assert np.abs(wl.subbox(a, org, s)[..., inner[0], inner[1], inner[2]] - b[..., inner[0], inner[1], inner[2]]).max() < 1e-15
+
+
+# ------------------------------------------------------------------ advection of phi: direction, upwinding, order (Eq. 3, R12)
+def _circular_com(phi):
+    """Centre of mass of a periodic blob per axis (x, y, z) through the first Fourier mode (exact for a symmetric blob)."""
+    out = []
+    for ax in (2, 1, 0):
+        n = phi.shape[ax]
+        prof = phi.sum(axis=tuple(a for a in range(3) if a != ax))
+        th = 2 * np.pi * np.arange(n) / n
+        out.append(np.arctan2((prof * np.sin(th)).sum(), (prof * np.cos(th)).sum()) * n / (2 * np.pi))
+    return np.array(out)
+
+
+def test_phi_blob_translates_with_plus_u():
+    """PAPER.md:L61 (Eq. 3): d_t phi + u.grad phi = ... moves phi WITH +u.  A tanh blob (R = 7, W = 4) in a uniform flow
+    u = (0.05, -0.02, 0.03) with sigma = 0 and equal densities (uniform flow is then an exact fixed point of the LB part)
+    must have its centre of mass displaced by u t after t = 100 steps (within 1 % of the smallest component) and stay
+    bounded; also catches a face flux differenced along the wrong axis."""
+    n, R, t = 32, 7.0, 100
+    uvec = np.array([0.05, -0.02, 0.03])
+    p = dict(tau=0.8, two_phase=1, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.05, width=4.0)
+    phi0 = wl.droplet_phi(n, R)
+    u0 = np.empty((3, n, n, n))
+    for al in range(3):
+        u0[al] = uvec[al]
+    o = oracle.Oracle(n, n, n, **p)
+    o.init(np.ones((n, n, n)), u0, phi0)
+    c0 = _circular_com(phi0)
+    o.step(t)
+    _, u, phi = o.moments()
+    assert np.abs(u - u0).max() < 1e-13                        # the carrier flow stays uniform
+    shift = (_circular_com(phi) - c0 + n / 2) % n - n / 2
+    assert np.abs(shift - uvec * t).max() < 0.01 * np.abs(uvec * t).min(), (shift, uvec * t)
+    assert phi.min() > -1e-3 and phi.max() < 1 + 1e-3
+    assert abs(o.diagnostics()["sum_phi"] / phi0.sum() - 1) < 1e-12
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("sign", [+1.0, -1.0])
+def test_phi_advection_one_step_is_minus_u_dphi_at_fifth_order(axis, sign):
+    """With D = 0 (mobility = 0 is legal: kappa = 4D/delta = 0) one forward-Euler step of Eq. 3 in a uniform flow is
+    phi(t+1) - phi(t) = -u d_a phi, the flux difference of the finite-difference WENO5 reconstruction (PAPER.md:L67,
+    R12), which approximates the derivative of a smooth profile to fifth order: error / k ~ k^5.  Pins the SIGN of the
+    advective term, the axis each face flux belongs to, and the order (wrong candidate / weight constants give 3), for
+    both upwind stencils.  (A multi-step refinement study cannot show more than first order: the integrator is
+    forward Euler, R13.)"""
+    errs = []
+    uval = sign * 0.04
+    for n in (16, 32, 64):
+        shape = [4, 4, 4]
+        shape[2 - axis] = n                                   # arrays are [z][y][x]; axis 0 = x
+        nz, ny, nx = shape
+        k = 2 * np.pi / n
+        coord = np.arange(n, dtype=float)
+        prof = 0.5 + 0.3 * np.sin(k * coord + 0.4)
+        bshape = [1, 1, 1]
+        bshape[2 - axis] = n
+        phi0 = np.ascontiguousarray(np.broadcast_to(prof.reshape(bshape), shape))
+        u0 = np.zeros((3, nz, ny, nx))
+        u0[axis] = uval
+        p = dict(tau=0.8, two_phase=1, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0, width=4.0)
+        o = oracle.Oracle(nx, ny, nz, **p)
+        o.init(np.ones(shape), u0, phi0)
+        o.step(1)
+        _, _, phi1 = o.moments()
+        dphi = ((phi1 - phi0) / (-uval)).reshape(-1, n) if axis == 0 else np.moveaxis((phi1 - phi0) / (-uval), 2 - axis, -1).reshape(-1, n)
+        exact = 0.3 * k * np.cos(k * coord + 0.4)
+        errs.append(np.abs(dphi - exact[None, :]).mean() / k)  # L1: WENO-JS drops to third order AT critical points only
+    o1, o2 = np.log2(errs[0] / errs[1]), np.log2(errs[1] / errs[2])
+    assert errs[0] < 2e-3 and o1 > 4.0 and o2 > 4.0, (errs, o1, o2)
+
+
+def test_phi_advection_is_upwind_biased():
+    """R12: the face value is reconstructed from the UPWIND side (`uf >= 0` takes cells x-2..x+2 for the face x+1/2).
+    On a marginally resolved wave (4 points per wavelength, D = 0) the upwind-biased fifth-order stencil is dissipative,
+    the downwind-biased one (the flipped test) amplifies: after 40 steps at |u| = 0.05 the L2 norm of the fluctuation
+    has decreased, for both signs of u."""
+    n = 32
+    x = np.arange(n, dtype=float)
+    prof = 0.5 + 0.05 * np.sin(2 * np.pi * x / 4)
+    shape = (4, 4, n)
+    phi0 = np.ascontiguousarray(np.broadcast_to(prof, shape))
+    p = dict(tau=0.8, two_phase=1, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0, width=4.0)
+    for uval in (0.05, -0.05):
+        u0 = np.zeros((3,) + shape)
+        u0[0] = uval
+        o = oracle.Oracle(n, 4, 4, **p)
+        o.init(np.ones(shape), u0, phi0)
+        o.step(40)
+        _, _, phi = o.moments()
+        amp0, amp1 = np.linalg.norm(phi0 - 0.5), np.linalg.norm(phi - 0.5)
+        assert 0.5 * amp0 < amp1 < 0.995 * amp0, (uval, amp0, amp1)
+
+
+# ------------------------------------------------------------------ F^nu on a prescribed shear (PAPER.md:L104 read as R9, L94)
+@pytest.mark.parametrize("pstar", [0.0, 1.0])
+def test_viscous_correction_force_on_prescribed_shear(pstar):
+    """Populations are prescribed in second-order Hermite space, f_i = f_i^eq(p*, m) + w_i H_i:a / (2 cs4) with
+    a = -cs2 tau (d_a u_b + d_b u_a) of a known smooth velocity m, rho(phi) a smooth wave, sigma = 0,
+    no body force.  By the moment identities of P2/P3, sum_i f_i c c = p* cs2 I + m m + a, so R9's force is
+      F^nu_a = -((tau-1/2)/tau) [a_ab + m_a m_b - ut_a ut_b] d_b rho,  ut = m + F^p/(2 rho),  F^p = -p* cs2 grad rho,
+    and for p* = 0 (no F^p) it reduces to  nu (d_a u_b + d_b u_a) d_b rho  exactly -- the reduction SURVEY R9 quotes.
+    The oracle's stored acceleration A = (F^p + F^nu)/rho is compared with this closed form; grad rho uses the lattice
+    stencil's plane-wave symbol (P5).  A wrong contraction index, prefactor, sign, or a dropped p* cs2 delta term fails."""
+    n, tau, rl, rg = 12, 0.9, 10.0, 1.0
+    nu = CS2 * (tau - 0.5)
+    c, w = oracle.lattice()
+    k = 2 * np.pi / n
+    ax = np.arange(n, dtype=float)
+    Z, Y, X = np.meshgrid(ax, ax, ax, indexing="ij")
+    amp = np.array([[0.0, 0.011, -0.007], [0.013, 0.0, 0.005], [-0.009, 0.006, 0.0]])   # amp[b][a]: u_b += amp sin(k x_a + ..)
+    diag = np.array([0.004, -0.008, 0.003])
+    pos = (X, Y, Z)
+    m = np.zeros((3, n, n, n))
+    du = np.zeros((3, 3, n, n, n))                    # du[a][b] = d_a u_b
+    for b in range(3):
+        for a in range(3):
+            coef = diag[b] if a == b else amp[b][a]
+            ph = k * pos[a] + 0.3 * (a + 1) + 0.5 * b
+            m[b] += coef * np.sin(ph)
+            du[a][b] += coef * k * np.cos(ph)
+    a_t = -CS2 * tau * (du + np.transpose(du, (1, 0, 2, 3, 4)))
+    kv = k * np.array([1, 2, -1])
+    phase = kv[0] * X + kv[1] * Y + kv[2] * Z + 0.7
+    phi = 0.5 + 0.25 * np.sin(phase)
+    s3 = (2 + np.cos(kv)) / 3
+    gphi = np.stack([np.sin(kv[al]) * np.prod(np.delete(s3, al)) * 0.25 * np.cos(phase) for al in range(3)])
+    rho = rg + (rl - rg) * phi
+    drho = (rl - rg) * gphi
+    # populations in Hermite space (numpy, from the lattice table only)
+    f = np.empty((27, n, n, n))
+    for i in range(27):
+        cu = sum(c[i][al] * m[al] for al in range(3))
+        H = np.outer(c[i], c[i]) - CS2 * np.eye(3)
+        huu = sum(H[al, be] * m[al] * m[be] for al in range(3) for be in range(3))
+        ha = sum(H[al, be] * a_t[al][be] for al in range(3) for be in range(3))
+        f[i] = w[i] * (pstar + cu / CS2 + huu / (2 * CS2 ** 2)) + w[i] * ha / (2 * CS2 ** 2)
+    p = dict(tau=tau, two_phase=1, rho_l=rl, rho_g=rg, sigma=0.0, mobility=0.05, width=4.0)
+    o = oracle.Oracle(n, n, n, **p)
+    o.init(np.full((n, n, n), pstar), np.zeros((3, n, n, n)), phi)
+    o.set_populations(f)
+    o.moments()
+    A = o.accel()
+    Fp = -pstar * CS2 * drho
+    ut = m + Fp / (2 * rho)
+    expect = np.zeros((3, n, n, n))
+    for al in range(3):
+        for be in range(3):
+            expect[al] += -((tau - 0.5) / tau) * (a_t[al][be] + m[al] * m[be] - ut[al] * ut[be]) * drho[be]
+    expect = (expect + Fp) / rho
+    assert np.abs(A - expect).max() < 1e-15 + 1e-13 * np.abs(expect).max(), np.abs(A - expect).max()
+    if pstar == 0.0:                                   # the continuum form of SURVEY R9 / PAPER.md:L94
+        visc = np.zeros((3, n, n, n))
+        for al in range(3):
+            for be in range(3):
+                visc[al] += nu * (du[al][be] + du[be][al]) * drho[be]
+        assert np.abs(A - visc / rho).max() < 1e-15 + 1e-13 * np.abs(visc / rho).max()
+        assert np.abs(visc / rho).max() > 1e-4         # the force is really there
