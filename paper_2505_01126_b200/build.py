@@ -14,7 +14,7 @@ ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libacclb.so"
 SOURCES = [CSRC / "acclb.cu"]
-HEADERS = [CSRC / "d3q27.cuh", CSRC / "stencils.cuh", CSRC / "twophase.cuh", CSRC / "pipeline.cuh", ROOT / "include" / "acclb.h"]
+HEADERS = [CSRC / "d3q27.cuh", CSRC / "stencils.cuh", CSRC / "twophase.cuh", ROOT / "include" / "acclb.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -7,9 +7,10 @@
 //                                                                                     PAPER.md:L75-92 (Eqs. 4-7)
 //   k_allen_cahn (two-phase) conservative Allen-Cahn, flux-form WENO5 + lattice stencils, forward Euler (a8)
 //                                                                                     PAPER.md:L61-67 (Eq. 3)
-// These three are the one-node-per-thread kernels (single-phase default; two-phase variant 1).  The default two-phase
-// step is k_lb_tp + k_advect (twophase.cuh: shared-memory tiles marching along z, TMA / cp.async staging); variant 2 is
-// the persistent L2-pipeline kernel k_step_tp (pipeline.cuh).
+// These three are the one-node-per-thread kernels (single-phase default; two-phase variant 1, kept as an in-library
+// cross-check of the tiled path).  The default two-phase step is the fused k_lb_tp + k_seam (twophase.cuh: shared-memory
+// tiles marching along z, TMA / cp.async staging, u and r never written to HBM); variant 2 is round 1's two-kernel form
+// k_lb_tp<unfused> + k_advect, kept for A/B measurements.
 // State: post-collision, not yet streamed populations f*_i(x) in SoA [z][i][y][x], double-buffered (A/B), so the
 // pull f_i(x,t) = f*_i(x - c_i, t-1) reads shifted rows and every store is aligned; phi double-buffered.
 // No CPU fallback, no library kernels: everything the path computes runs in the kernels of this file.
@@ -48,7 +49,15 @@ template <typename ST> struct Pop;
 template <> struct Pop<double> {
   static __device__ __forceinline__ double from_storage(double v, int) { return v; }
   static __device__ __forceinline__ double load(const double* p, int) { return __ldcs(p); }
+#if defined(XP_ST_CG)
+  static __device__ __forceinline__ void store(double* p, int, double v) { __stcg(p, v); }
+#elif defined(XP_ST_WT)
+  static __device__ __forceinline__ void store(double* p, int, double v) { __stwt(p, v); }
+#elif defined(XP_ST_DEF)
+  static __device__ __forceinline__ void store(double* p, int, double v) { *p = v; }
+#else
   static __device__ __forceinline__ void store(double* p, int, double v) { __stcs(p, v); }
+#endif
 };
 template <> struct Pop<float> {
   static __device__ __forceinline__ double from_storage(float v, int i) { return (double)v + w_of(i); }
@@ -433,7 +442,6 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
 }  // namespace acclb
 
 #include "twophase.cuh"
-#include "pipeline.cuh"
 
 // ================================================================================================== host / ABI
 using namespace acclb;
@@ -454,9 +462,8 @@ struct accLB_ctx {
   double* acc;
   CUtensorMap tmap[2];  // populations A / B as rank-3 tensors (x, y, z * 27 + i) for the TMA pull of k_lb_tp
   int tmap_ok;          // 0: tensor maps unavailable (shape the map cannot describe, or no driver entry point)
-  double* rings;  // pipeline ring buffers: n(3) | g,c(4) | r | u(3) | fz, a few planes each (two-phase)
-  int* sync;      // pipeline counters: ticket | done[4][nz + 4]
-  int pipe_grid;  // resident blocks of k_step_tp
+  Seams seams;    // u on the seams of the tile columns (k_lb_tp<FUSED> -> k_seam)
+  int lz;         // planes per block of the z-marching kernels
   double* stage;  // [5 n] rho | u(3) | phi, host_staging only
   int cur;        // f[cur], phi[cur] hold the current state
   long long step;
@@ -487,7 +494,8 @@ struct LaunchScope {
     }
   }
 };
-enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_STEP = 6 };
+enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_LB_TP = 6,
+       KIND_SEAM = 7, KIND_ADVECT = 8 };
 
 static thread_local char g_err[512] = "";
 
@@ -514,36 +522,11 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
   return true;
 }
 
-struct Carve {
-  size_t f, phi, u, r, nrm, tabs, acc, rings, sync, stage, total;
-};
-static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
-  const size_t n = (size_t)nx * ny * nz;
-  Carve c;
-  c.f = align256(27 * n * (p->store_fp32 ? 4 : 8));
-  c.phi = p->two_phase ? align256(n * 8) : 0;
-  c.u = p->two_phase ? align256(3 * n * 8) : 0;
-  c.r = p->two_phase ? align256(n * 8) : 0;
-  c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
-  c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
-  c.acc = align256(16 * 8);
-  c.rings = p->two_phase ? align256((size_t)PIPE_RING_DOUBLES * nx * ny * 8) : 0;
-  c.sync = p->two_phase ? align256((size_t)(1 + 4 * (nz + 4)) * 4) : 0;
-  c.stage = p->host_staging ? align256(5 * n * 8) : 0;
-  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.rings + c.sync + c.stage;
-  return c;
-}
-
-#define CK(call)                                                                                      \
-  do {                                                                                                \
-    cudaError_t e_ = (call);                                                                          \
-    if (e_ != cudaSuccess) return fail(ACCLB_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
-  } while (0)
-
-static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
-
 // Tile shapes of the two-phase kernels.
-constexpr int LBT_TX = 32, LBT_TY = 8, LBT_MINB = 2;
+#ifndef XP_MINB
+#define XP_MINB 2
+#endif
+constexpr int LBT_TX = 32, LBT_TY = 8, LBT_MINB = XP_MINB;
 constexpr int ADV_TX = 32, ADV_TY = 8;
 
 // Planes per block along z: enough blocks to load every SM a few times over, chunks of equal length, and no
@@ -558,20 +541,73 @@ static int planes_per_block(int nx, int ny, int nz, int tx, int ty) {
   return (nz + chunks - 1) / chunks;
 }
 
-template <typename ST>
+struct Carve {
+  size_t f, phi, u, r, nrm, tabs, acc, sx, sy, sz, stage, total;
+};
+static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
+  const size_t n = (size_t)nx * ny * nz;
+  Carve c;
+  c.f = align256(27 * n * (p->store_fp32 ? 4 : 8));
+  c.phi = p->two_phase ? align256(n * 8) : 0;
+  c.u = p->two_phase ? align256(3 * n * 8) : 0;
+  c.r = p->two_phase ? align256(n * 8) : 0;
+  c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
+  c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
+  c.acc = align256(16 * 8);
+  const size_t ntx = (nx + LBT_TX - 1) / LBT_TX, nty = (ny + LBT_TY - 1) / LBT_TY;
+  const int lz = planes_per_block(nx, ny, nz, LBT_TX, LBT_TY);
+  const size_t nchunk = (nz + lz - 1) / lz;
+  c.sx = p->two_phase ? align256((size_t)nz * ny * 2 * ntx * 8) : 0;
+  c.sy = p->two_phase ? align256((size_t)nz * 2 * nty * nx * 8) : 0;
+  c.sz = p->two_phase ? align256(2 * nchunk * (size_t)ny * nx * 8) : 0;
+  c.stage = p->host_staging ? align256(5 * n * 8) : 0;
+  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.sx + c.sy + c.sz + c.stage;
+  return c;
+}
+
+#define CK(call)                                                                                      \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) return fail(ACCLB_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+template <typename ST, bool FUSED>
 static int launch_lb_tp(accLB_ctx* s, int c, int d) {
-  using T = GeoTile<ST, LBT_TX, LBT_TY>;
-  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB>;
+  using T = GeoTile<ST, LBT_TX, LBT_TY, FUSED>;
+  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB, FUSED>;
   static thread_local int configured_device = -1;
   if (configured_device != s->prm.device) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
     configured_device = s->prm.device;
   }
-  const int lz = planes_per_block(s->nx, s->ny, s->nz, LBT_TX, LBT_TY);
+  const int lz = s->lz;
   const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
-  LaunchScope ls(s, KIND_LB);
+  LaunchScope ls(s, KIND_LB_TP);
   kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], s->u, s->r,
-                                                        s->tabs, lz, s->tmap[c], s->tmap_ok);
+                                                        s->phi[d], s->seams, s->tabs, lz, s->tmap[c], s->tmap_ok);
+  return ACCLB_OK;
+}
+
+// The fluxes through the seam faces of the tile columns (k_seam: one launch per direction), after k_lb_tp<FUSED> of the
+// same step.
+static int launch_seam(accLB_ctx* s, int c, int d) {
+  const int nchunk = (s->nz + s->lz - 1) / s->lz;
+  const size_t nfx = (size_t)s->seams.ntx * s->ny * s->nz, nfy = (size_t)s->nx * s->seams.nty * s->nz,
+               nfz = (size_t)s->nx * s->ny * nchunk;
+  {
+    LaunchScope ls(s, KIND_SEAM);
+    k_seam<1><<<blocks_for(nfy, 128), 128, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, LBT_TY, s->seams.nty, (unsigned)nfy);
+  }
+  {
+    LaunchScope ls(s, KIND_SEAM);
+    k_seam<0><<<blocks_for(nfx, 128), 128, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, LBT_TX, s->seams.ntx, (unsigned)nfx);
+  }
+  {
+    LaunchScope ls(s, KIND_SEAM);
+    k_seam<2><<<blocks_for(nfz, 128), 128, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, s->lz, nchunk, (unsigned)nfz);
+  }
   return ACCLB_OK;
 }
 
@@ -585,52 +621,8 @@ static int launch_advect(accLB_ctx* s, int c, int d) {
   }
   const int lz = planes_per_block(s->nx, s->ny, s->nz, ADV_TX, ADV_TY);
   const dim3 grid((s->nx + ADV_TX - 1) / ADV_TX, (s->ny + ADV_TY - 1) / ADV_TY, (s->nz + lz - 1) / lz);
-  LaunchScope ls(s, KIND_AC);
+  LaunchScope ls(s, KIND_ADVECT);
   kern<<<grid, ADV_TX * ADV_TY, sizeof(T), s->stream>>>(s->kp, s->phi[c], s->u, s->r, s->phi[d], lz);
-  return ACCLB_OK;
-}
-
-// The two-phase step as one persistent pipeline kernel (pipeline.cuh).
-constexpr int PIPE_MINB = 3;
-
-template <typename ST>
-static int launch_step_tp(accLB_ctx* s, int c, int d) {
-  auto kern = k_step_tp<ST, PIPE_MINB>;
-  if (s->pipe_grid == 0) {
-    int per_sm = 0, sms = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PIPE_THREADS, 0));
-    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->prm.device));
-    if (per_sm < 1) return fail(ACCLB_ECUDA, "k_step_tp: no resident block fits an SM");
-    s->pipe_grid = per_sm * sms;
-  }
-  PipeArgs a;
-  a.P = s->kp;
-  a.fin = s->f[c];
-  a.fout = s->f[d];
-  a.phi = s->phi[c];
-  a.phi_new = s->phi[d];
-  a.tabs = s->tabs;
-  const size_t plane = (size_t)s->nx * s->ny;
-  double* w = s->rings;
-  a.ring_n = w; w += 3 * RING_N * plane;
-  a.ring_gc = w; w += 4 * RING_GC * plane;
-  a.ring_r = w; w += RING_R * plane;
-  a.ring_u = w; w += 3 * RING_U * plane;
-  a.ring_fz = w;
-  a.ticket = s->sync;
-  a.done = s->sync + 1;
-  a.tiles_x = (s->nx + PIPE_TX - 1) / PIPE_TX;
-  a.tiles_y = (s->ny + PIPE_TY - 1) / PIPE_TY;
-  a.tiles = a.tiles_x * a.tiles_y;
-  a.lb_items = (int)((plane + PIPE_THREADS - 1) / PIPE_THREADS);
-  a.per_macro = 3 * a.tiles + a.lb_items;
-  const long long total = (long long)(s->nz + 3 + LAG_ADV) * a.per_macro;
-  if (total >= 2000000000LL) return fail(ACCLB_EINVAL, "k_step_tp: too many work items");
-  a.total = (int)total;
-  CK(cudaMemsetAsync(s->sync, 0, (size_t)(1 + 4 * (s->nz + 4)) * 4, s->stream));
-  const int grid = (int)(total < s->pipe_grid ? total : s->pipe_grid);
-  LaunchScope ls(s, KIND_STEP);
-  kern<<<grid, PIPE_THREADS, 0, s->stream>>>(a);
   return ACCLB_OK;
 }
 
@@ -703,9 +695,12 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   s->nrm = p->two_phase ? (double*)w : nullptr; w += c.nrm;
   s->tabs = (double*)w; w += c.tabs;
   s->acc = (double*)w; w += c.acc;
-  s->rings = p->two_phase ? (double*)w : nullptr; w += c.rings;
-  s->sync = p->two_phase ? (int*)w : nullptr; w += c.sync;
-  s->pipe_grid = 0;
+  s->seams.sx = p->two_phase ? (double*)w : nullptr; w += c.sx;
+  s->seams.sy = p->two_phase ? (double*)w : nullptr; w += c.sy;
+  s->seams.sz = p->two_phase ? (double*)w : nullptr; w += c.sz;
+  s->seams.ntx = (nx + LBT_TX - 1) / LBT_TX;
+  s->seams.nty = (ny + LBT_TY - 1) / LBT_TY;
+  s->lz = planes_per_block(nx, ny, nz, LBT_TX, LBT_TY);
   s->stage = p->host_staging ? (double*)w : nullptr; w += c.stage;
   s->cur = 0; s->step = 0; s->launches = 0; s->variant = 0; s->profiling = 0;
 
@@ -791,14 +786,16 @@ int accLB_step(accLB_ctx* s, int nsteps) {
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
     if (s->prm.two_phase && s->variant == 0) {
-      // default: fused LB + geometry on z-marching tiles (k_lb_tp), then the advective phi update (k_advect)
-      int r = s->prm.store_fp32 ? launch_lb_tp<float>(s, c, d) : launch_lb_tp<double>(s, c, d);
+      // default: LB + geometry + advection fused on z-marching tiles (k_lb_tp), then the seam faces (k_seam)
+      int r = s->prm.store_fp32 ? launch_lb_tp<float, true>(s, c, d) : launch_lb_tp<double, true>(s, c, d);
       if (r) return r;
-      r = launch_advect(s, c, d);
+      r = launch_seam(s, c, d);
       if (r) return r;
     } else if (s->prm.two_phase && s->variant == 2) {
-      // variant 2: the whole step as one persistent pipeline kernel (k_step_tp, pipeline.cuh)
-      int r = s->prm.store_fp32 ? launch_step_tp<float>(s, c, d) : launch_step_tp<double>(s, c, d);
+      // variant 2: round 1's two-kernel form, u and r through HBM (k_lb_tp<unfused>, k_advect)
+      int r = s->prm.store_fp32 ? launch_lb_tp<float, false>(s, c, d) : launch_lb_tp<double, false>(s, c, d);
+      if (r) return r;
+      r = launch_advect(s, c, d);
       if (r) return r;
     } else if (s->prm.two_phase) {
       // variant 1: one node per thread, stencils straight from global memory (k_normal, k_lb, k_allen_cahn)

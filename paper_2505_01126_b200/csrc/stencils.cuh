@@ -111,32 +111,34 @@ __device__ __forceinline__ double div_pos(double a, double b) {
   return __fma_rn(__fma_rn(-b, q, a), r, q);
 }
 
-// Jiang-Shu WENO5 value at the face downwind of `c`, from the five upwind-ordered cell values (R12;
-// PAPER.md:L67, ref. [19]): candidates q_k, smoothness b_k, weights d_k / (eps + b_k)^2, d = (.1,.6,.3), eps = 1e-6.
-// The three weight divisions and the normalisation are folded into one division (div_pos) by multiplying through with
-// the product of the (eps + b_k)^2.  Every operation is an explicitly rounded intrinsic so that the two cells
-// sharing a face evaluate bit-identical fluxes (exact conservation of sum phi, R12).
-__device__ __forceinline__ double weno5_face(double a, double b, double c, double d, double e) {
-  const double k1312 = 13.0 / 12.0, sixth = 1.0 / 6.0, eps = 1e-6;
-  const double q0 = __dmul_rn(__fma_rn(11.0, c, __fma_rn(-7.0, b, __dmul_rn(2.0, a))), sixth);
-  const double q1 = __dmul_rn(__fma_rn(2.0, d, __fma_rn(5.0, c, -b)), sixth);
-  const double q2 = __dmul_rn(__fma_rn(5.0, d, __fma_rn(2.0, c, -e)), sixth);
-  const double s0 = __dadd_rn(__fma_rn(-2.0, b, a), c);          // a - 2b + c
-  const double t0 = __fma_rn(3.0, c, __fma_rn(-4.0, b, a));      // a - 4b + 3c
-  const double s1 = __dadd_rn(__fma_rn(-2.0, c, b), d);          // b - 2c + d
-  const double t1 = __dsub_rn(b, d);                             // b - d
-  const double s2 = __dadd_rn(__fma_rn(-2.0, d, c), e);          // c - 2d + e
-  const double t2 = __dadd_rn(__fma_rn(-4.0, d, __dmul_rn(3.0, c)), e);  // 3c - 4d + e
-  const double b0 = __fma_rn(k1312, __dmul_rn(s0, s0), __dmul_rn(0.25, __dmul_rn(t0, t0)));
-  const double b1 = __fma_rn(k1312, __dmul_rn(s1, s1), __dmul_rn(0.25, __dmul_rn(t1, t1)));
-  const double b2 = __fma_rn(k1312, __dmul_rn(s2, s2), __dmul_rn(0.25, __dmul_rn(t2, t2)));
-  const double r0 = __dadd_rn(eps, b0), r1 = __dadd_rn(eps, b1), r2 = __dadd_rn(eps, b2);
+// Jiang-Shu WENO5 (R12, ref. [19]) at the face downwind of `c`, from the five upwind-ordered cell values
+// a..e, written on the four differences d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d.  Returns face value MINUS c:
+//   candidates   q0 - c = (5 d2 - 2 d1)/6,  q1 - c = (d2 + 2 d3)/6,  q2 - c = (4 d3 - d4)/6
+//   smoothness   b0 = 13/12 (d2 - d1)^2 + 1/4 (3 d2 - d1)^2,  b1 = 13/12 (d3 - d2)^2 + 1/4 (d2 + d3)^2,
+//                b2 = 13/12 (d4 - d3)^2 + 1/4 (d4 - 3 d3)^2
+//   weights      d_k / (eps + b_k)^2, d = (.1,.6,.3), eps = 1e-6, normalised.
+// The same numbers as the textbook form up to rounding (12 b_k and 12 eps are used: a common factor of the three
+// (eps + b_k) drops out of the normalised weights), with a fifth fewer fp64 operations.  The three weight divisions and the
+// normalisation are folded into one division (div_pos) by multiplying through with the product of the (eps + b_k)^2.
+// Every operation is an explicitly rounded intrinsic so that the two cells sharing a face evaluate bit-identical
+// fluxes wherever a face is evaluated twice (k_seam): exact conservation of sum phi, R12.
+__device__ __forceinline__ double weno5_minus_c(double d1, double d2, double d3, double d4) {
+  const double eps12 = 12.0e-6;
+  const double s0 = __dsub_rn(d2, d1), t0 = __fma_rn(3.0, d2, -d1);
+  const double s1 = __dsub_rn(d3, d2), t1 = __dadd_rn(d2, d3);
+  const double s2 = __dsub_rn(d4, d3), t2 = __fma_rn(-3.0, d3, d4);
+  const double r0 = __fma_rn(13.0, __dmul_rn(s0, s0), __fma_rn(3.0, __dmul_rn(t0, t0), eps12));  // 12 (eps + b0)
+  const double r1 = __fma_rn(13.0, __dmul_rn(s1, s1), __fma_rn(3.0, __dmul_rn(t1, t1), eps12));
+  const double r2 = __fma_rn(13.0, __dmul_rn(s2, s2), __fma_rn(3.0, __dmul_rn(t2, t2), eps12));
   const double e0 = __dmul_rn(r0, r0), e1 = __dmul_rn(r1, r1), e2 = __dmul_rn(r2, r2);
   const double n0 = __dmul_rn(0.1, __dmul_rn(e1, e2));
   const double n1 = __dmul_rn(0.6, __dmul_rn(e0, e2));
   const double n2 = __dmul_rn(0.3, __dmul_rn(e0, e1));
-  const double num = __fma_rn(n2, q2, __fma_rn(n1, q1, __dmul_rn(n0, q0)));
-  const double den = __dadd_rn(__dadd_rn(n0, n1), n2);
+  const double x0 = __fma_rn(5.0, d2, __dmul_rn(-2.0, d1));  // 6 (q0 - c)
+  const double x1 = __fma_rn(2.0, d3, d2);                   // 6 (q1 - c)
+  const double x2 = __fma_rn(4.0, d3, -d4);                  // 6 (q2 - c)
+  const double num = __fma_rn(n2, x2, __fma_rn(n1, x1, __dmul_rn(n0, x0)));
+  const double den = __dmul_rn(6.0, __dadd_rn(__dadd_rn(n0, n1), n2));
   return div_pos(num, den);
 }
 
@@ -151,7 +153,8 @@ __device__ __forceinline__ double face_flux(double uL, double uR, double pm2, do
   const double c = pos ? p0 : pp1;
   const double d = pos ? pp1 : p0;
   const double e = pos ? pp2 : pm1;
-  return __dmul_rn(uf, weno5_face(a, b, c, d, e));
+  const double w = weno5_minus_c(__dsub_rn(b, a), __dsub_rn(c, b), __dsub_rn(d, c), __dsub_rn(e, d));
+  return __dmul_rn(uf, __dadd_rn(c, w));
 }
 
 }  // namespace acclb

@@ -1,15 +1,24 @@
 // Two-phase hot path on shared-memory tiles, device side (sm_100a).  Part of the CUDA product path.
 //
-// One two-phase step is two kernels:
-//   k_lb_tp     rows a1-a7 + the phi-only part of a8.  A block owns a TX x TY column of nodes and marches along z.
+// One two-phase step is the fused kernel k_lb_tp<FUSED = true> plus the small seam kernel k_seam:
+//   k_lb_tp     rows a1-a8.  A block owns a TX x TY column of nodes and marches along z.
 //               Per plane it stages phi (halo 2) in shared memory, derives the interface normal n, the sharpening flux
 //               q = phi (1 - phi) n and |grad phi| ONCE per node of the tile + 1 rim (they are needed at the 26
 //               neighbours by div n and div q), then every thread does its node: kappa_c = div n,
 //               F^s, F^p, F^nu (Eq. 8), pull-stream, moments, Hermite coefficient, regularized reconstruction, aligned
-//               store (Eqs. 6-7), and writes u (needed by the advection) and r = D lap phi - kappa div q (Eq. 3).
-//   k_advect    the advective part of a8: phi+ = phi + (-sum_e (Phi_e(x) - Phi_e(x - e)) + r), Phi = u_f WENO5(phi) in
-//               flux form (R12).  Every face flux is computed once per face (shared memory for x / y
-//               faces, a register carried along the z march for z faces), so sum phi is conserved to rounding.
+//               store (Eqs. 6-7), u and r = D lap phi - kappa div q (Eq. 3).
+//               FUSED: u and r never leave the SM.  One plane behind the node update the block evaluates the advective
+//               WENO5 fluxes Phi_e = u_f WENO5(phi) (R12) through every face INSIDE its tile column
+//               (x faces: neighbour lane; y faces: shared memory; z faces: carried along the march) and writes
+//               phi(t+1) = phi + r - sum_e (Phi_e(x) - Phi_e(x - e)) without the faces on the tile's seams, whose second
+//               velocity belongs to another block; the velocities on the seams go to three thin strips (2.6 B per node).
+//   k_seam      adds the fluxes through the seam faces (x = multiples of TX, y = multiples of TY, z = multiples of lz:
+//               5 % of all faces) to the cells on either side, from the strips and phi(t).  Every cell gathers its own
+//               seam faces with the same explicitly rounded instruction sequence, so a face's flux has identical bits
+//               on both sides and sum phi is conserved to rounding (R12) without atomics.
+//   FUSED = false + k_advect is the round-1 two-kernel form (u, r through HBM), kept as variant 2 for comparison:
+//   k_advect    the advective part of a8: phi+ = phi + (-sum_e (Phi_e(x) - Phi_e(x - e)) + r); every face flux is
+//               computed once per face (shared memory for x / y faces, a register carried along z for z faces).
 // Periodic boundaries are index wraps when the tiles are filled (PAPER.md:L114's halo exchange is not needed).
 // Staging: the 27 pulled populations of the next plane arrive by TMA (27 tiled cp.async.bulk.tensor box loads issued by
 // one thread, mbarrier completion) in tiles away from the y rim, by one cp.async per thread and population elsewhere; phi,
@@ -73,6 +82,13 @@ __device__ __forceinline__ void cp_async_f64(double* smem, const double* gmem) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
 }
+// 16 bytes, L2 only (no L1 line is allocated): the staging copies of this file.  With 2 x 100 KB of shared memory per SM the
+// L1 is down to 28 KB, and 8-byte cp.async.ca copies that each allocate a 128-byte L1 line (a phi plane's halo columns,
+// the edge elements of the pull) thrashed it: 10.9 -> 12.1 ms for 10 KB more shared memory per block (measured).
+__device__ __forceinline__ void cp_async_16(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
 template <int N>
 __device__ __forceinline__ void cp_async_wait_but() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
@@ -82,7 +98,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 //   The D3Q27 stencil weights factorise, w_i = W(cx) W(cy) W(cz) / 216 with W = (1,4,1), so every lattice stencil of
 //   PAPER.md:L104 is evaluated separably: a z combination per (x,y) column first (Sz = (1,4,1), Dz = (+1,0,-1)), then a
 //   3 x 3 stencil in the plane.  Same numbers as the 27-term sums up to rounding order.
-template <typename ST, int TX, int TY>
+template <typename ST, int TX, int TY, bool FUSED>
 struct GeoTile {
   // Landing zone of the pulled populations of the next plane.  For interior tiles the TMA writes population i's TX x TY box
   // of rows y0 - c_iy, plane z - c_iz, UNSHIFTED in x (TMA needs 16-byte aligned box starts, and a window widened to the next
@@ -95,32 +111,55 @@ struct GeoTile {
   unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
-  double raw[4][PY][PX];  // ring of raw phi planes zc-1, zc, zc+1 and zc+2 (landing, cp.async)
+  static constexpr int NR = FUSED ? 5 : 4;
+  alignas(16) double raw[NR][PY][PX];  // ring of raw phi planes (zc-2,) zc-1, zc, zc+1 and zc+2 (landing, cp.async)
   double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
   double ftab[2][64];     // sin / cos force table entries of this block's planes (lz <= 64): the streaming pulls evict
                           // everything from L1, so a per-plane __ldg of the table would wait for L2 every plane
   double ftx[2][TX], fty[2][TY];  // the same for the tile's columns and rows (kept here rather than in 8 registers)
+  // FUSED advection (row a8), one plane behind the node update:
+  static constexpr int NA = FUSED ? TX * TY : 1;
+  double ux[NA], uy[NA];  // u_x, u_y of the plane updated last (read by the neighbour lane / row)
+  double fy[NA];          // flux through the y face above the node
+  double e[NA];           // own slot: phi + r of the plane updated last
+  double col[3][NA];      // own slots: phi of the three planes older than the ring (z-face window)
+#ifdef XP_PAD
+  double pad_[XP_PAD];
+#endif
+  double acc[NA];         // own slot: phi(t+1) of the previous advected plane, still missing its upper z flux
+};
+
+// Velocity on the seams of the tile columns, written by k_lb_tp<FUSED> and read by k_seam (layouts in accLB_create):
+//   sx[(z ny + y) 2 ntx + 2 bx + s]   u_x at the first (s = 0) / last (s = 1) column of tile column bx
+//   sy[(z 2 nty + 2 by + s) nx + x]   u_y at the first / last row of tile row by
+//   sz[((2 bz + s) ny + y) nx + x]    u_z at the first / last plane of z chunk bz
+struct Seams {
+  double* sx;
+  double* sy;
+  double* sz;
+  int ntx, nty;  // tile columns / rows
 };
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
 // Iteration zc: phi(zc+1) has landed, fetch phi(zc+2) | derive n, q (tile + 1) and g, |g|, lap (own node, kept in
-// registers) on plane zc from the raw planes zc-1, zc, zc+1 | plane sums of plane zc, then the node update of plane
-// z = zc - 1, whose z combinations need planes zc-2 .. zc (carried in registers).
-// The 27 populations a thread pulls for plane z are fetched with cp.async into the thread's own shared-memory slots while
+// registers) on plane zc from the raw planes zc-1, zc, zc+1; FUSED: advective fluxes of plane zc-2 | plane sums of plane
+// zc, then the node update of plane z = zc - 1, whose z combinations need planes zc-2 .. zc (carried in registers).
+// The 27 populations a thread pulls for plane z are fetched with TMA / cp.async into shared memory while
 // the block is still busy with plane z-1 and with the geometry of plane z: the HBM latency of the pull hides under the
 // fp64 work instead of stalling every warp at the top of the node update, and no register holds a load in flight.
-template <typename ST, int TX, int TY, int MINB>
+template <typename ST, int TX, int TY, int MINB, bool FUSED>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
-        double* __restrict__ uout, double* __restrict__ rout, const double* __restrict__ tabs, int lz,
-        const __grid_constant__ CUtensorMap tmap_fin, int use_tma) {
-  using T = GeoTile<ST, TX, TY>;
+        double* __restrict__ uout, double* __restrict__ rout, double* __restrict__ phi_new, Seams SM,
+        const double* __restrict__ tabs, int lz, const __grid_constant__ CUtensorMap tmap_fin, int use_tma) {
+  using T = GeoTile<ST, TX, TY, FUSED>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
   constexpr int NT = TX * TY;
-  constexpr int RIM2 = T::PX * T::PY - NT;  // staging items besides the thread's own node
+  constexpr int NR = T::NR;
   constexpr int RIM1 = T::NX * T::NY - NT;  // derive items besides the thread's own node
-  static_assert(RIM2 <= NT && RIM1 <= NT, "at most one rim item per thread");
+  static_assert(RIM1 <= NT, "at most one rim item per thread");
+  static_assert(TX == 32 || !FUSED, "FUSED: one warp per tile row (x-face fluxes travel by warp shuffle)");
   const Grid& G = P.G;
   const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * lz;
@@ -129,14 +168,14 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const bool active = x < G.nx && y < G.ny;
   const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
 
-  // rim item of the staging pass: the tid-th element of the PY x PX plane that is not an own node
-  int r2 = -1;  // linear index j * PX + i in a phi plane
+  // staging item of this thread: the tid-th aligned pair of doubles of a PY x PX phi plane (tile + halo 2; x0 and nx are
+  // even, so a pair never straddles the periodic wrap), copied with one 16-byte cp.async
+  constexpr int PAIRS = T::PX / 2 * T::PY;
+  static_assert(PAIRS <= NT && T::PX % 2 == 0, "one staging pair per thread");
+  int r2 = -1;  // linear index j * PX + i of the pair's first element
   unsigned r2off = 0;
-  if (tid < RIM2) {
-    int j, i;
-    if (tid < 2 * T::PX) { j = tid / T::PX; i = tid % T::PX; }                                   // rows 0, 1
-    else if (tid < 4 * T::PX) { j = TY + tid / T::PX; i = tid % T::PX; }                         // rows PY-2, PY-1
-    else { const int e = tid - 4 * T::PX; j = 2 + e / 4; i = (e & 3) < 2 ? (e & 3) : TX + (e & 3); }  // columns
+  if (tid < PAIRS) {
+    const int j = tid / (T::PX / 2), i = 2 * (tid % (T::PX / 2));
     r2 = j * T::PX + i;
     r2off = (unsigned)pmod(y0 - 2 + j, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 2 + i, G.nx);
   }
@@ -163,18 +202,27 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   // per-thread copy instructions, no address registers held by copies in flight, no L1 allocation.  The two edge lanes of
   // a row fetch the 9 + 9 elements outside the boxes themselves.  All other tiles: one 8-byte cp.async per thread and
   // population.  Either way population i of thread (tx, ty) ends up at *slot(i).
-  const bool fast = use_tma && x0 + TX <= G.nx && y0 >= 1 && y0 + TY + 1 <= G.ny;  // block-uniform
+  const bool fast = sizeof(ST) == 8 && use_tma && x0 + TX <= G.nx && y0 >= 1 && y0 + TY + 1 <= G.ny;  // block-uniform
   // three per-thread bases, one per c_ix, so that slot(i) is base + a compile-time offset
   ST* const sl_c = &S.fpop[0][ty * TX + tx];
-  ST* const sl_p = tx == 0 ? &S.fpop[0][NT + ty] : sl_c - 1;       // c_ix = +1: element x - 1
-  ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + ty] : sl_c + 1;  // c_ix = -1: element x + 1
+  // (fast tiles: the slab's tail holds, per tile row, the aligned pair (x0-2, x0-1) for c_ix = +1 / (x0+TX, x0+TX+1) for -1)
+  ST* const sl_p = tx == 0 ? &S.fpop[0][NT + (fast ? 2 * ty + 1 : ty)] : sl_c - 1;       // c_ix = +1: element x - 1
+  ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + (fast ? 2 * ty : ty)] : sl_c + 1;      // c_ix = -1: element x + 1
   auto slot = [&](int i) -> ST* { return (cx_of(i) == 0 ? sl_c : cx_of(i) == 1 ? sl_p : sl_m) + i * T::SLAB; };
-  auto tma_pull = [&](int z) {  // called by thread 0 only
+  // The TMA issue is spread over the block's warps (lane 0 of warp w issues boxes w, w + 8, ...): one thread issuing all 27
+  // made its warp arrive late at the next barrier in every iteration.  Thread 0 arms the mbarrier with the byte count.
+  auto tma_pull = [&](int z) {  // called by lane 0 of every warp, after the block-wide hand-over of the landing zone
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    mbar_arrive_expect_tx(&S.fbar, (unsigned)(Q * NT * sizeof(ST)));
+    if (tid == 0) mbar_arrive_expect_tx(&S.fbar, (unsigned)(Q * NT * sizeof(ST)));
     const int zs[3] = {wrap_dec(z, G.nz) * Q, z * Q, wrap_inc(z, G.nz) * Q};
 #pragma unroll
-    for (int i = 0; i < Q; ++i) tma_load_box(&S.fpop[i][0], &tmap_fin, x0, y0 - cy_of(i), zs[1 - cz_of(i)] + i, &S.fbar);
+    for (int k = 0; k < (Q + TY - 1) / TY; ++k) {
+      const int i = ty + k * TY;
+      if (i < Q) {
+        const int cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
+        tma_load_box(&S.fpop[i][0], &tmap_fin, x0, y0 - cy, (cz < 0 ? zs[2] : cz > 0 ? zs[0] : zs[1]) + i, &S.fbar);
+      }
+    }
   };
   if (fast) {
     if (tid == 0) {
@@ -182,17 +230,31 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (tid == 0) tma_pull(z0);
+    if (tx == 0) tma_pull(z0);
+  }
+  // fast tiles: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
+  // c_ix = -1) are fetched by lanes 0..17 of the row's warp, one 16-byte cp.async each (the aligned pair that holds the
+  // element), into the tail of the slabs
+  static_assert(sizeof(ST) == 8 || TY * 16 <= 128, "edge pairs fit the slab tail");
+  unsigned e_off = 0;  // i * plane + row + column of this lane's edge pair
+  if (fast && tx < 18) {
+    const int m = tx < 9 ? tx : tx - 9;
+    const int e_i = 3 * m + (tx < 9 ? 2 : 0), cy = m % 3 - 1;
+    e_off = (unsigned)e_i * plane + (cy < 0 ? yrow[2] : cy > 0 ? yrow[0] : yrow[1]) + (unsigned)(tx < 9 ? pmod(x0 - 2, G.nx) : pmod(x0 + TX, G.nx));
   }
   auto prefetch_pull = [&](int z) {
-    if (fast && tx != 0 && tx != TX - 1) {  // the boxes are on their way (thread 0, after the block-wide hand-over)
+    if (fast) {  // the boxes are on their way (lane 0 of every warp, after the block-wide hand-over)
+      if (tx < 18) {
+        const int m = tx < 9 ? tx : tx - 9;  // population 3 m + 2 (c_ix = +1) or 3 m (c_ix = -1), c_iz = m / 3 - 1
+        const ST* sl = pop_slab(fin, G, m < 3 ? wrap_inc(z, G.nz) : m >= 6 ? wrap_dec(z, G.nz) : z);
+        cp_async_16(&S.fpop[3 * m + (tx < 9 ? 2 : 0)][NT + 2 * ty], sl + e_off);
+      }
       cp_async_commit();
       return;
     }
     const ST* slab[3] = {pop_slab(fin, G, wrap_dec(z, G.nz)), pop_slab(fin, G, z), pop_slab(fin, G, wrap_inc(z, G.nz))};
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
-      if (fast && !((cx_of(i) == 1 && tx == 0) || (cx_of(i) == -1 && tx == TX - 1))) continue;
       const unsigned off = (unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)];
       cp_async_pop<(int)sizeof(ST)>(slot(i), slab[1 - cz_of(i)] + off);
     }
@@ -200,11 +262,11 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   };
   // Per-thread cp.async groups alternate phi plane | populations, every thread commits both in every iteration (an
   // empty group where it has nothing to fetch), so "all but the newest group" is always the one needed next.
-  // phi(zc+2) lands in the 4th ring plane one iteration before it is combined: its latency hides under plane zc.
+  // phi(zc+2) lands in the ring one iteration before it is combined: its latency hides under plane zc.
+  // Ring slots: plane z0 - 2 + j lives in slot j mod NR.
   {
     const double* s2 = phi + (size_t)pmod(z0, G.nz) * plane;
-    cp_async_f64(&S.raw[2][0][0] + o2, s2 + o2off);
-    if (r2 >= 0) cp_async_f64(&S.raw[2][0][0] + r2, s2 + r2off);
+    if (r2 >= 0) cp_async_16(&S.raw[2][0][0] + r2, s2 + r2off);
     cp_async_commit();
   }
   if (active) prefetch_pull(z0);
@@ -216,16 +278,17 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     const double* s1 = phi + (size_t)pmod(z0 - 1, G.nz) * plane;
     double* d0 = &S.raw[0][0][0];
     double* d1 = &S.raw[1][0][0];
-    d0[o2] = __ldg(s0 + o2off);
-    d1[o2] = __ldg(s1 + o2off);
     if (r2 >= 0) {
-      d0[r2] = __ldg(s0 + r2off);
-      d1[r2] = __ldg(s1 + r2off);
+      *reinterpret_cast<double2*>(d0 + r2) = __ldg(reinterpret_cast<const double2*>(s0 + r2off));
+      *reinterpret_cast<double2*>(d1 + r2) = __ldg(reinterpret_cast<const double2*>(s1 + r2off));
     }
   }
   double an0 = 0.0, an1 = 0.0, bn0 = 0.0, bn1 = 0.0;  // plane sums of n at planes zc-2, zc-1
   double aq0 = 0.0, aq1 = 0.0, bq0 = 0.0, bq1 = 0.0;  // plane sums of q
   double gp[3] = {0.0, 0.0, 0.0}, gnp = 0.0, lapp = 0.0;  // g, |g|, lap phi of the own node at plane zc-1
+  // FUSED: u_z at planes zc-3, zc-2; slot of plane zc-5 in the column history S.col (planes zc-5, zc-4, zc-3)
+  double uzm = 0.0, uzc = 0.0;
+  int cj = 0;
   // x-, y- and z-dependent table entries of the body force (R20) of this tile and chunk
   if (P.force_type != 0) {
     if (ty == 0) { S.ftx[0][tx] = __ldg(tabs + xw); S.ftx[1][tx] = __ldg(tabs + G.nx + xw); }
@@ -238,28 +301,35 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   __syncthreads();
 
   int zq2 = pmod(z0 + 1, G.nz);  // wrapped zc + 2, carried (no integer division in the march)
-  for (int zc = z0 - 1; zc <= z1; ++zc) {
-    const int it = zc - (z0 - 1);  // 0, 1, 2, ...
+  int sb = 0;                    // element offset of the ring slot of plane zc-1 (slot = it mod NR), carried
+  const int zc_last = FUSED ? z1 + 1 : z1;  // FUSED: one more iteration to advect the last plane
+  for (int zc = z0 - 1; zc <= zc_last; ++zc) {
+    // ring planes zc-1+k, k = 0..3 (k = NR-1 is plane zc-2 when FUSED), as element offsets from S.raw; sb is carried
+    constexpr int PSZ = T::PX * T::PY;
+    auto ring = [&](int k) -> double* {
+      int o = sb + k * PSZ;
+      if (o >= NR * PSZ) o -= NR * PSZ;
+      return &S.raw[0][0][0] + o;
+    };
     // ---- phi(zc+1) has landed (this thread's own elements); fetch phi(zc+2)
     {
       cp_async_wait_but<1>();
-      double* rn = &S.raw[(it + 3) & 3][0][0];        // plane zc+2: its slot held plane zc-2, last read before the
-                                                      // previous iteration's second barrier
+      double* rn = ring(3);  // plane zc+2: its slot held plane zc+2-NR, last read before the previous iteration's
+                             // second barrier
       if (zc < z1) {
         const double* src = phi + (size_t)zq2 * plane;
-        cp_async_f64(rn + o2, src + o2off);
-        if (r2 >= 0) cp_async_f64(rn + r2, src + r2off);
+        if (r2 >= 0) cp_async_16(rn + r2, src + r2off);
       }
       cp_async_commit();
       zq2 = wrap_inc(zq2, G.nz);
     }
     __syncthreads();
     // ---- derive n, q (tile + 1 rim) and g, |g|, lap (own node) on plane zc           PAPER.md:L61, L104; R17
-    double gc[3], gnc, lapc;
-    {
-      const double* rm = &S.raw[it & 3][0][0];        // plane zc-1
-      const double* rc = &S.raw[(it + 1) & 3][0][0];  // plane zc
-      const double* rp = &S.raw[(it + 2) & 3][0][0];  // plane zc+1
+    double gc[3] = {0.0, 0.0, 0.0}, gnc = 0.0, lapc = 0.0;
+    if (!FUSED || zc <= z1) {
+      const double* rm = ring(0);  // plane zc-1
+      const double* rc = ring(1);  // plane zc
+      const double* rp = ring(2);  // plane zc+1
       auto derive = [&](int j, int i, bool own_node) {  // (j, i) in the NY x NX plane; centre (j+1, i+1) in a phi plane
         constexpr int PX = T::PX;
         const int b = j * PX + i;
@@ -300,17 +370,70 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         }
       };
       derive(ty + 1, tx + 1, true);
+#ifndef XP_NORIM
       if (r1 >= 0) derive(r1 / T::NX, r1 % T::NX, false);
+#endif
+    }
+    // ---- FUSED a8: advective fluxes of plane p = zc - 2 through the faces inside the tile column (R12)
+    //   x face (x, x+1): own u_x and the neighbour lane's;  y face (y, y+1): u_y of the row above (shared memory);
+    //   z face (p-1, p): u_z carried along the march.  Faces on the tile's seams are left to k_seam.
+    const int pz = zc - 2;
+#ifdef XP_NOADV
+    const bool adv = false;
+#else
+    const bool adv = FUSED && pz >= z0;  // block-uniform; pz <= z1 - 1 because zc <= z1 + 1
+#endif
+    double Tp = 0.0;                     // phi(t+1) of plane pz, accumulated
+    if (FUSED) {
+      const double* rq = ring(NR - 1);                   // plane zc-2 = pz, tile + halo 2
+      const double php = rq[o2];
+      if (adv) {
+        constexpr int PX = T::PX;
+        const bool xseam = tx == TX - 1 || x + 1 >= G.nx;  // the face to the right is a seam (or the thread idle)
+        const bool yseam = ty == TY - 1 || y + 1 >= G.ny;
+        const double* row = rq + (ty + 2) * PX + tx;       // phi(x-2 .. x+3) of the own row
+#ifdef XP_NOFLUX
+#define face_flux(a,b,c,d,e,f,g,h) ((a)+(b)+(c)+(d)+(e)+(f)+(g)+(h))
+#endif
+        double Fx = face_flux(S.ux[tid], S.ux[xseam ? tid : tid + 1], row[0], row[1], row[2], row[3], row[4], row[5]);
+        Fx = xseam ? 0.0 : Fx;
+        double Fxl = __shfl_up_sync(0xffffffffu, Fx, 1);
+        Fxl = tx == 0 ? 0.0 : Fxl;
+        const double* col = rq + ty * PX + (tx + 2);       // phi(y-2 .. y+3) of the own column
+        double Fy = face_flux(S.uy[tid], S.uy[yseam ? tid : tid + TX], col[0], col[PX], col[2 * PX], col[3 * PX], col[4 * PX],
+                              col[5 * PX]);
+        Fy = yseam ? 0.0 : Fy;
+        S.fy[tid] = Fy;
+        // z face (pz-1, pz): phi(pz-3 .. pz+2) = the column history, then planes zc-2, zc-1, zc of the ring
+        const int cj1 = cj == 2 ? 0 : cj + 1, cj2 = cj1 == 2 ? 0 : cj1 + 1;
+        double Fz = face_flux(uzm, uzc, S.col[cj][tid], S.col[cj1][tid], S.col[cj2][tid], php, ring(0)[o2], ring(1)[o2]);
+        Fz = pz == z0 ? 0.0 : Fz;
+        if (pz > z0 && active) __stcs(phi_new + (size_t)(pz - 1) * plane + o2off, S.acc[tid] - Fz);  // plane pz-1 is complete
+        Tp = S.e[tid] - (Fx - Fxl) - Fy + Fz;
+#ifdef XP_NOFLUX
+#undef face_flux
+#endif
+      }
+      S.col[cj][tid] = php;  // plane zc-2 replaces plane zc-5
+      cj = cj == 2 ? 0 : cj + 1;
     }
     __syncthreads();
+    if (adv) {
+      Tp += ty == 0 ? 0.0 : S.fy[tid - TX];
+      if (pz == z1 - 1) {  // the face above the chunk's last plane is a seam
+        if (active) __stcs(phi_new + (size_t)pz * plane + o2off, Tp);
+      } else {
+        S.acc[tid] = Tp;
+      }
+    }
     // ---- plane sums of plane zc at the own node:  a = Dx Sy v_x + Sx Dy v_y,  b = Sx Sy v_z
-    double an2, bn2, aq2, bq2;
-    {
+    double an2 = 0.0, bn2 = 0.0, aq2 = 0.0, bq2 = 0.0;
+    if (!FUSED || zc <= z1) {
       constexpr int NX = T::NX;
-      auto plane_sums = [&](int c0, double& a, double& b) {
-        const double* vx = &S.nq[c0][ty][tx];
-        const double* vy = &S.nq[c0 + 1][ty][tx];
-        const double* vz = &S.nq[c0 + 2][ty][tx];
+      auto plane_sums = [&](int c0_, double& a, double& b) {
+        const double* vx = &S.nq[c0_][ty][tx];
+        const double* vy = &S.nq[c0_ + 1][ty][tx];
+        const double* vz = &S.nq[c0_ + 2][ty][tx];
         const double ax = fma(4.0, vx[NX + 2] - vx[NX], (vx[2] - vx[0]) + (vx[2 * NX + 2] - vx[2 * NX]));
         const double ay = fma(4.0, vy[2 * NX + 1] - vy[1], (vy[2 * NX] - vy[0]) + (vy[2 * NX + 2] - vy[2]));
         a = ax + ay;
@@ -323,8 +446,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       plane_sums(3, aq2, bq2);
     }
     const int z = zc - 1;
-    if (!(z >= z0 && active)) cp_async_commit();
-    if (z >= z0 && active) {
+    double uz_new = 0.0;
+    if (!(z >= z0 && z < z1 && active)) cp_async_commit();
+    if (z >= z0 && z < z1 && active) {
       // a1-a2: the pulled populations have landed in this thread's slots; moments, then refill the slots for plane z+1
       cp_async_wait_but<1>();
       if (fast) mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
@@ -332,17 +456,19 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
       if (fast) {  // every warp has read its 27 values out of the landing zone: refill it for plane z+1
         __syncthreads();
-        if (tid == 0 && z + 1 < z1) tma_pull(z + 1);
+        if (tx == 0 && z + 1 < z1) tma_pull(z + 1);
       }
       if (z + 1 < z1) prefetch_pull(z + 1);
       else cp_async_commit();
       // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
       const double kc = (1.0 / 72.0) * (fma(4.0, an1, an0 + an2) + (bn2 - bn0));
       const double divq = (1.0 / 72.0) * (fma(4.0, aq1, aq0 + aq2) + (bq2 - bq0));
-      const double phi0 = S.raw[it & 3][ty + 2][tx + 2];  // plane zc-1 = z
+      const double phi0 = ring(0)[o2];  // plane zc-1 = z
 
       const unsigned k = (unsigned)z * plane + yrow[1] + (unsigned)xs[1];
-      rout[k] = P.D * lapp - P.kappa * divq;  // phi-only part of Eq. 3
+      const double rr = P.D * lapp - P.kappa * divq;  // phi-only part of Eq. 3
+      if (FUSED) S.e[tid] = phi0 + rr;
+      else rout[k] = rr;
 
       // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
       double Fb[3] = {0.0, 0.0, 0.0};
@@ -362,14 +488,86 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       double A[3], rho;
       accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, true, A, rho);
       const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
-      uout[k] = u[0];
-      uout[G.n + k] = u[1];
-      uout[2u * G.n + k] = u[2];
+      if (FUSED) {
+        S.ux[tid] = u[0];
+        S.uy[tid] = u[1];
+        uz_new = u[2];
+        // velocities on the seams of this tile column, for k_seam
+#ifndef XP_NOSEAMW
+        // (every strip has fewer elements than the grid has nodes: 32-bit indices)
+        const unsigned ix = ((unsigned)z * (unsigned)G.ny + (unsigned)y) * (unsigned)(2 * SM.ntx) + 2u * blockIdx.x;
+        if (tx == 0) SM.sx[ix] = u[0];
+        if (tx == TX - 1 || x == G.nx - 1) SM.sx[ix + 1] = u[0];
+        const unsigned iy = ((unsigned)z * (unsigned)(2 * SM.nty) + 2u * blockIdx.y) * (unsigned)G.nx + (unsigned)x;
+        if (ty == 0) SM.sy[iy] = u[1];
+        if (ty == TY - 1 || y == G.ny - 1) SM.sy[iy + (unsigned)G.nx] = u[1];
+        if (z == z0) SM.sz[(2u * blockIdx.z) * plane + o2off] = u[2];
+        if (z == z1 - 1) SM.sz[(2u * blockIdx.z + 1u) * plane + o2off] = u[2];
+#endif
+      } else {
+        uout[k] = u[0];
+        uout[(size_t)G.n + k] = u[1];
+        uout[2 * (size_t)G.n + k] = u[2];
+      }
       collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + (yrow[1] + (unsigned)xs[1]), plane);
     }
     an0 = an1; an1 = an2; bn0 = bn1; bn1 = bn2;
     aq0 = aq1; aq1 = aq2; bq0 = bq1; bq1 = bq2;
     gp[0] = gc[0]; gp[1] = gc[1]; gp[2] = gc[2]; gnp = gnc; lapp = lapc;
+    uzm = uzc; uzc = uz_new;
+    sb = sb + PSZ == NR * PSZ ? 0 : sb + PSZ;
+  }
+}
+
+// a8 on the seams of the tile columns of k_lb_tp<FUSED> (R12).  A face is a seam when its two cells
+// belong to different tile columns / z chunks: x faces in front of x = TX b, y faces in front of y = TY b, z faces in
+// front of z = lz b (b = 0 is the periodic wrap).  One launch per direction DIR (0: x, 1: y, 2: z), one thread per seam
+// face: it evaluates the flux once from the two strip velocities and phi(t) and adds it to phi(t+1) of the cell behind
+// the face (+) and of the cell in front (-), so sum phi is conserved to rounding.  All updates of one cell within a launch
+// come from one thread (a tile only one cell thick gets both of its faces from the thread of its lower face), and the
+// three launches are ordered on the stream: no atomics, bitwise reproducible.
+template <int DIR>
+__global__ void __launch_bounds__(128) k_seam(KP P, const double* __restrict__ phi, double* __restrict__ phi_new, Seams SM,
+                                              int tile, int ntile, unsigned nfaces) {
+  const Grid& G = P.G;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nfaces) return;
+  const size_t plane = (size_t)G.nx * (size_t)G.ny;
+  const int n = DIR == 0 ? G.nx : DIR == 1 ? G.ny : G.nz;  // extent along DIR
+  int x, y, z, b;                                           // b: tile whose first cell lies behind the face
+  if (DIR == 0) {
+    b = (int)(t % (unsigned)ntile);
+    const unsigned r = t / (unsigned)ntile;
+    y = (int)(r % (unsigned)G.ny); z = (int)(r / (unsigned)G.ny); x = b * tile;
+  } else if (DIR == 1) {
+    x = (int)(t % (unsigned)G.nx);
+    const unsigned r = t / (unsigned)G.nx;
+    b = (int)(r % (unsigned)ntile); z = (int)(r / (unsigned)ntile); y = b * tile;
+  } else {
+    x = (int)(t % (unsigned)G.nx);
+    const unsigned r = t / (unsigned)G.nx;
+    y = (int)(r % (unsigned)G.ny); b = (int)(r / (unsigned)G.ny); z = b * tile;
+  }
+  const int c0 = b * tile;  // coordinate along DIR of the cell behind the face
+  const int bp = b == 0 ? ntile - 1 : b - 1, bn = b == ntile - 1 ? 0 : b + 1;
+  const size_t stride = DIR == 0 ? 1 : DIR == 1 ? (size_t)G.nx : plane;
+  const size_t base = (size_t)z * plane + (size_t)y * G.nx + x - (size_t)c0 * stride;  // cell with coordinate 0 along DIR
+  auto ph = [&](int k) { return __ldg(phi + base + (size_t)wrap_add(c0, k, n) * stride); };
+  auto vel = [&](int bb, int s) {  // strip velocity of tile bb, first (s = 0) or last (s = 1) cell along DIR
+    if (DIR == 0) return __ldg(SM.sx + ((size_t)z * G.ny + y) * (size_t)(2 * SM.ntx) + 2 * bb + s);
+    if (DIR == 1) return __ldg(SM.sy + ((size_t)z * (size_t)(2 * SM.nty) + 2 * bb + s) * G.nx + x);
+    return __ldg(SM.sz + (size_t)(2 * bb + s) * plane + (size_t)y * G.nx + x);
+  };
+  const double p_3 = ph(-3), p_2 = ph(-2), p_1 = ph(-1), p0 = ph(0), p1 = ph(1), p2 = ph(2);
+  const double uLs = vel(bp, 1), uRs = vel(b, 0);
+  const double F = face_flux(uLs, uRs, p_3, p_2, p_1, p0, p1, p2);
+  double dR = F;
+  if (min(tile, n - c0) == 1) dR -= face_flux(vel(b, 1), vel(bn, 0), p_2, p_1, p0, p1, p2, ph(3));  // one-cell tile: its upper face too
+  double* const cR = phi_new + base + (size_t)c0 * stride;
+  *cR = *cR + dR;
+  if (min(tile, n - bp * tile) > 1) {
+    double* const cL = phi_new + base + (size_t)wrap_add(c0, -1, n) * stride;
+    *cL = *cL - F;
   }
 }
 

@@ -293,11 +293,11 @@ def test_launch_count_and_errors(acclb):
     sim2 = gpu_sim(acclb, cfg2)
     c0 = sim2.launch_count
     sim2.step(4)
-    assert sim2.launch_count - c0 == 8         # fused LB + geometry on tiles, then advection
+    assert sim2.launch_count - c0 == 16        # LB + geometry + advection fused on tiles, then the seam faces (x, y, z)
     sim2.set_variant(2)
     c0 = sim2.launch_count
     sim2.step(4)
-    assert sim2.launch_count - c0 == 4         # variant 2: the whole two-phase step as one persistent pipeline kernel
+    assert sim2.launch_count - c0 == 8         # variant 2: round 1's two-kernel form (u, r through HBM)
     sim2.set_variant(1)
     c0 = sim2.launch_count
     sim2.step(4)
@@ -311,8 +311,8 @@ def test_launch_count_and_errors(acclb):
 @pytest.mark.parametrize("variant", [1, 2])
 @pytest.mark.parametrize("ratio", [1.0, 10.0])
 def test_variant_kernels_match_oracle_and_default(acclb, ratio, variant):
-    """Variant 1 (one node per thread, stencils from global memory), variant 2 (one persistent pipeline kernel) and the
-    default tiled two-kernel path agree with the oracle and with each other to rounding; switching variants in mid-run is
+    """Variant 1 (one node per thread, stencils from global memory), variant 2 (tiled, u and r through HBM) and the
+    default fused path agree with the oracle and with each other to rounding; switching variants in mid-run is
     allowed."""
     cfg = wl.make_config("droplet", n=40, density_ratio=ratio)
     a, b, o = gpu_sim(acclb, cfg), gpu_sim(acclb, cfg), cpu_sim(cfg)
