@@ -460,8 +460,9 @@ struct accLB_ctx {
   double* nrm;
   double* tabs;
   double* acc;
-  CUtensorMap tmap[2];  // populations A / B as rank-3 tensors (x, y, z * 27 + i) for the TMA pull of k_lb_tp
-  int tmap_ok;          // 0: tensor maps unavailable (shape the map cannot describe, or no driver entry point)
+  CUtensorMap tmap[2];      // populations A / B as rank-3 tensors (x, y, z * 27 + i) for the TMA pull of k_lb_tp<FAST>,
+  CUtensorMap tmap_row[2];  // box TX x TY x 1, and box TX x 1 x 1 (single rows: tiles on the periodic y rim)
+  int tmap_ok;              // 0: no FAST path (tile shape does not divide the box, fp32 storage, no driver entry point)
   Seams seams;    // u on the seams of the tile columns (k_lb_tp<FUSED> -> k_seam)
   int lz;         // planes per block of the z-marching kernels
   double* stage;  // [5 n] rho | u(3) | phi, host_staging only
@@ -573,10 +574,10 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
 
 static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
-template <typename ST, bool FUSED>
+template <typename ST, bool FUSED, bool FAST>
 static int launch_lb_tp(accLB_ctx* s, int c, int d) {
   using T = GeoTile<ST, LBT_TX, LBT_TY, FUSED>;
-  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB, FUSED>;
+  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB, FUSED, FAST>;
   static thread_local int configured_device = -1;
   if (configured_device != s->prm.device) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
@@ -586,8 +587,16 @@ static int launch_lb_tp(accLB_ctx* s, int c, int d) {
   const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
   LaunchScope ls(s, KIND_LB_TP);
   kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], s->u, s->r,
-                                                        s->phi[d], s->seams, s->tabs, lz, s->tmap[c], s->tmap_ok);
+                                                        s->phi[d], s->seams, s->tabs, lz, s->tmap[c], s->tmap_row[c]);
   return ACCLB_OK;
+}
+
+// FAST (all tiles full, TMA pull) when the tensor maps exist and the tile shape divides the box; fp64 storage only.
+template <bool FUSED>
+static int launch_lb_tp_any(accLB_ctx* s, int c, int d) {
+  if (s->prm.store_fp32) return launch_lb_tp<float, FUSED, false>(s, c, d);
+  if (s->tmap_ok) return launch_lb_tp<double, FUSED, true>(s, c, d);
+  return launch_lb_tp<double, FUSED, false>(s, c, d);
 }
 
 // The fluxes through the seam faces of the tile columns (k_seam: one launch per direction), after k_lb_tp<FUSED> of the
@@ -642,14 +651,17 @@ static int make_tensor_maps(accLB_ctx* s) {
   }
   if (s->prm.store_fp32) return 0;  // measured: with 128-byte rows the per-thread cp.async pull is faster (9.5 vs 9.9 ms)
   const size_t es = 8;
-  if (((size_t)s->nx * es) % 16 != 0 || s->nx < LBT_TX || s->ny < LBT_TY) return 0;
+  if (s->nx % LBT_TX != 0 || s->ny % LBT_TY != 0) return 0;  // FAST: every tile full
   const cuuint64_t dims[3] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny, (cuuint64_t)27 * s->nz};
   const cuuint64_t strides[2] = {(cuuint64_t)s->nx * es, (cuuint64_t)s->nx * s->ny * es};
-  const cuuint32_t box[3] = {LBT_TX, LBT_TY, 1}, estr[3] = {1, 1, 1};
+  const cuuint32_t box[3] = {LBT_TX, LBT_TY, 1}, row[3] = {LBT_TX, 1, 1}, estr[3] = {1, 1, 1};
   for (int b = 0; b < 2; ++b) {
-    const CUresult r = ((encode_t)fn)(&s->tmap[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, s->f[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = ((encode_t)fn)(&s->tmap[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, s->f[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return 0;
+    r = ((encode_t)fn)(&s->tmap_row[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, s->f[b], dims, strides, row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return 0;
   }
   return 1;
@@ -787,13 +799,13 @@ int accLB_step(accLB_ctx* s, int nsteps) {
     const int c = s->cur, d = c ^ 1;
     if (s->prm.two_phase && s->variant == 0) {
       // default: LB + geometry + advection fused on z-marching tiles (k_lb_tp), then the seam faces (k_seam)
-      int r = s->prm.store_fp32 ? launch_lb_tp<float, true>(s, c, d) : launch_lb_tp<double, true>(s, c, d);
+      int r = launch_lb_tp_any<true>(s, c, d);
       if (r) return r;
       r = launch_seam(s, c, d);
       if (r) return r;
     } else if (s->prm.two_phase && s->variant == 2) {
       // variant 2: round 1's two-kernel form, u and r through HBM (k_lb_tp<unfused>, k_advect)
-      int r = s->prm.store_fp32 ? launch_lb_tp<float, false>(s, c, d) : launch_lb_tp<double, false>(s, c, d);
+      int r = launch_lb_tp_any<false>(s, c, d);
       if (r) return r;
       r = launch_advect(s, c, d);
       if (r) return r;

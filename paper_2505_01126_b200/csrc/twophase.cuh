@@ -147,11 +147,15 @@ struct Seams {
 // The 27 populations a thread pulls for plane z are fetched with TMA / cp.async into shared memory while
 // the block is still busy with plane z-1 and with the geometry of plane z: the HBM latency of the pull hides under the
 // fp64 work instead of stalling every warp at the top of the node update, and no register holds a load in flight.
-template <typename ST, int TX, int TY, int MINB, bool FUSED>
+// FAST (fp64 storage, nx a multiple of TX, ny a multiple of TY, tensor maps available): every tile is full and pulls by
+// TMA; no thread is idle and no per-thread wrap tables are kept.  Otherwise every tile pulls with per-thread cp.async.
+template <typename ST, int TX, int TY, int MINB, bool FUSED, bool FAST>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
         double* __restrict__ uout, double* __restrict__ rout, double* __restrict__ phi_new, Seams SM,
-        const double* __restrict__ tabs, int lz, const __grid_constant__ CUtensorMap tmap_fin, int use_tma) {
+        const double* __restrict__ tabs, int lz, const __grid_constant__ CUtensorMap tmap_fin,
+        const __grid_constant__ CUtensorMap tmap_row) {
+  static_assert(!FAST || sizeof(ST) == 8, "the TMA pull is for fp64 storage");
   using T = GeoTile<ST, TX, TY, FUSED>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
@@ -165,7 +169,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * lz;
   const int z1 = min(z0 + lz, G.nz);
   const int x = x0 + tx, y = y0 + ty;
-  const bool active = x < G.nx && y < G.ny;
+  const bool active = FAST || (x < G.nx && y < G.ny);
   const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
 
   // staging item of this thread: the tid-th aligned pair of doubles of a PY x PX phi plane (tile + halo 2; x0 and nx are
@@ -191,27 +195,34 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     r1 = r1j * T::NX + r1i;
   }
 
-  const int xw = pmod(x, G.nx), yw = pmod(y, G.ny);
-  const int xs[3] = {wrap_dec(xw, G.nx), xw, wrap_inc(xw, G.nx)};
-  const unsigned yrow[3] = {(unsigned)wrap_dec(yw, G.ny) * (unsigned)G.nx, (unsigned)yw * (unsigned)G.nx,
-                            (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx};
-
   // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1).
-  // Tiles whose shifted rows stay inside the box in y (no periodic wrap: TMA zero-fills out of bounds) and that are full
-  // width: ONE thread issues 27 tiled TMA loads (cp.async.bulk.tensor), completion counted in bytes on an mbarrier; no
-  // per-thread copy instructions, no address registers held by copies in flight, no L1 allocation.  The two edge lanes of
-  // a row fetch the 9 + 9 elements outside the boxes themselves.  All other tiles: one 8-byte cp.async per thread and
-  // population.  Either way population i of thread (tx, ty) ends up at *slot(i).
-  const bool fast = sizeof(ST) == 8 && use_tma && x0 + TX <= G.nx && y0 >= 1 && y0 + TY + 1 <= G.ny;  // block-uniform
+  // FAST: 27 tiled TMA loads per plane (cp.async.bulk.tensor, issued by lane 0 of the block's warps, three or four boxes
+  // each), completion counted in bytes on an mbarrier; no per-thread copy instructions, no address registers held by
+  // copies in flight, no L1 allocation.  Lanes 0..17 of a row fetch the 9 + 9 elements per row outside the boxes.
+  // Otherwise: one 8-byte cp.async per thread and population.  Either way population i of thread (tx, ty) is at *slot(i).
+  constexpr bool fast = FAST;
+  // Tiles on the y rim of the box: the rows shifted by c_iy wrap around, and TMA zero-fills out-of-bounds rows instead of
+  // wrapping, so these tiles fetch the populations with c_iy != 0 row by row (TX x 1 boxes, every row wrapped on its own,
+  // lanes 0..TY-1 of the issuing warp).
+  const bool yrim = FAST && (y0 == 0 || y0 + TY >= G.ny);  // block-uniform
+  // wrap tables of the per-thread pull (not FAST)
+  int xs[3] = {0, 0, 0};
+  unsigned yrow[3] = {0, 0, 0};
+  if (!FAST) {
+    const int xw = pmod(x, G.nx), yw = pmod(y, G.ny);
+    xs[0] = wrap_dec(xw, G.nx); xs[1] = xw; xs[2] = wrap_inc(xw, G.nx);
+    yrow[0] = (unsigned)wrap_dec(yw, G.ny) * (unsigned)G.nx; yrow[1] = (unsigned)yw * (unsigned)G.nx;
+    yrow[2] = (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx;
+  }
   // three per-thread bases, one per c_ix, so that slot(i) is base + a compile-time offset
   ST* const sl_c = &S.fpop[0][ty * TX + tx];
-  // (fast tiles: the slab's tail holds, per tile row, the aligned pair (x0-2, x0-1) for c_ix = +1 / (x0+TX, x0+TX+1) for -1)
+  // (FAST: the slab's tail holds, per tile row, the aligned pair (x0-2, x0-1) for c_ix = +1 / (x0+TX, x0+TX+1) for -1)
   ST* const sl_p = tx == 0 ? &S.fpop[0][NT + (fast ? 2 * ty + 1 : ty)] : sl_c - 1;       // c_ix = +1: element x - 1
   ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + (fast ? 2 * ty : ty)] : sl_c + 1;      // c_ix = -1: element x + 1
   auto slot = [&](int i) -> ST* { return (cx_of(i) == 0 ? sl_c : cx_of(i) == 1 ? sl_p : sl_m) + i * T::SLAB; };
-  // The TMA issue is spread over the block's warps (lane 0 of warp w issues boxes w, w + 8, ...): one thread issuing all 27
-  // made its warp arrive late at the next barrier in every iteration.  Thread 0 arms the mbarrier with the byte count.
-  auto tma_pull = [&](int z) {  // called by lane 0 of every warp, after the block-wide hand-over of the landing zone
+  // The TMA issue is spread over the block's warps (warp w issues boxes w, w + TY, ...): one thread issuing all 27 made
+  // its warp arrive late at the next barrier in every iteration.  Thread 0 arms the mbarrier with the byte count.
+  auto tma_pull = [&](int z) {  // called by lanes 0..TY-1 of every warp, after the block-wide hand-over of the landing zone
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (tid == 0) mbar_arrive_expect_tx(&S.fbar, (unsigned)(Q * NT * sizeof(ST)));
     const int zs[3] = {wrap_dec(z, G.nz) * Q, z * Q, wrap_inc(z, G.nz) * Q};
@@ -220,7 +231,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const int i = ty + k * TY;
       if (i < Q) {
         const int cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
-        tma_load_box(&S.fpop[i][0], &tmap_fin, x0, y0 - cy, (cz < 0 ? zs[2] : cz > 0 ? zs[0] : zs[1]) + i, &S.fbar);
+        const int slab = (cz < 0 ? zs[2] : cz > 0 ? zs[0] : zs[1]) + i;
+        if (yrim && cy != 0) tma_load_box(&S.fpop[i][tx * TX], &tmap_row, x0, pmod(y0 - cy + tx, G.ny), slab, &S.fbar);
+        else if (tx == 0) tma_load_box(&S.fpop[i][0], &tmap_fin, x0, y0 - cy, slab, &S.fbar);
       }
     }
   };
@@ -230,9 +243,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (tx == 0) tma_pull(z0);
+    if (tx < TY) tma_pull(z0);
   }
-  // fast tiles: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
+  // FAST: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
   // c_ix = -1) are fetched by lanes 0..17 of the row's warp, one 16-byte cp.async each (the aligned pair that holds the
   // element), into the tail of the slabs
   static_assert(sizeof(ST) == 8 || TY * 16 <= 128, "edge pairs fit the slab tail");
@@ -240,10 +253,11 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   if (fast && tx < 18) {
     const int m = tx < 9 ? tx : tx - 9;
     const int e_i = 3 * m + (tx < 9 ? 2 : 0), cy = m % 3 - 1;
-    e_off = (unsigned)e_i * plane + (cy < 0 ? yrow[2] : cy > 0 ? yrow[0] : yrow[1]) + (unsigned)(tx < 9 ? pmod(x0 - 2, G.nx) : pmod(x0 + TX, G.nx));
+    e_off = (unsigned)e_i * plane + (unsigned)pmod(y - cy, G.ny) * (unsigned)G.nx +
+            (unsigned)(tx < 9 ? pmod(x0 - 2, G.nx) : pmod(x0 + TX, G.nx));
   }
   auto prefetch_pull = [&](int z) {
-    if (fast) {  // the boxes are on their way (lane 0 of every warp, after the block-wide hand-over)
+    if (fast) {  // the boxes are on their way (after the block-wide hand-over)
       if (tx < 18) {
         const int m = tx < 9 ? tx : tx - 9;  // population 3 m + 2 (c_ix = +1) or 3 m (c_ix = -1), c_iz = m / 3 - 1
         const ST* sl = pop_slab(fin, G, m < 3 ? wrap_inc(z, G.nz) : m >= 6 ? wrap_dec(z, G.nz) : z);
@@ -291,6 +305,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   int cj = 0;
   // x-, y- and z-dependent table entries of the body force (R20) of this tile and chunk
   if (P.force_type != 0) {
+    const int xw = pmod(x, G.nx), yw = pmod(y, G.ny);
     if (ty == 0) { S.ftx[0][tx] = __ldg(tabs + xw); S.ftx[1][tx] = __ldg(tabs + G.nx + xw); }
     if (tx == 0) { S.fty[0][ty] = __ldg(tabs + 2 * G.nx + yw); S.fty[1][ty] = __ldg(tabs + 2 * G.nx + G.ny + yw); }
     if (tid < z1 - z0) {
@@ -456,7 +471,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
       if (fast) {  // every warp has read its 27 values out of the landing zone: refill it for plane z+1
         __syncthreads();
-        if (tx == 0 && z + 1 < z1) tma_pull(z + 1);
+        if (tx < TY && z + 1 < z1) tma_pull(z + 1);
       }
       if (z + 1 < z1) prefetch_pull(z + 1);
       else cp_async_commit();
@@ -465,7 +480,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const double divq = (1.0 / 72.0) * (fma(4.0, aq1, aq0 + aq2) + (bq2 - bq0));
       const double phi0 = ring(0)[o2];  // plane zc-1 = z
 
-      const unsigned k = (unsigned)z * plane + yrow[1] + (unsigned)xs[1];
+      const unsigned k = (unsigned)z * plane + o2off;
       const double rr = P.D * lapp - P.kappa * divq;  // phi-only part of Eq. 3
       if (FUSED) S.e[tid] = phi0 + rr;
       else rout[k] = rr;
@@ -509,7 +524,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         uout[(size_t)G.n + k] = u[1];
         uout[2 * (size_t)G.n + k] = u[2];
       }
-      collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + (yrow[1] + (unsigned)xs[1]), plane);
+      collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
     }
     an0 = an1; an1 = an2; bn0 = bn1; bn1 = bn2;
     aq0 = aq1; aq1 = aq2; bq0 = bq1; bq1 = bq2;
