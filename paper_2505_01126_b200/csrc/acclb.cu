@@ -536,7 +536,7 @@ static int planes_per_block(int nx, int ny, int nz, int tx, int ty) {
   const long long tiles = (long long)((nx + tx - 1) / tx) * ((ny + ty - 1) / ty);
   long long lz = (long long)nz * tiles / (148LL * 12LL);
   if (lz < 8) lz = 8;
-  if (lz > 64) lz = 64;
+  if (lz > LZ_MAX) lz = LZ_MAX;
   if (lz > nz) lz = nz;
   const int chunks = (int)((nz + lz - 1) / lz);
   return (nz + chunks - 1) / chunks;

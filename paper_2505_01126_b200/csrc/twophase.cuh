@@ -25,7 +25,15 @@
 // u, r planes arrive by cp.async one plane ahead.
 #pragma once
 
+#include <type_traits>
+
 namespace acclb {
+
+#ifdef XP_LZ
+constexpr int LZ_MAX = XP_LZ;
+#else
+constexpr int LZ_MAX = 64;  // planes per block along z, at most
+#endif
 
 __device__ __forceinline__ int pmod(int a, int n) {
   int r = a % n;
@@ -114,7 +122,7 @@ struct GeoTile {
   static constexpr int NR = FUSED ? 5 : 4;
   alignas(16) double raw[NR][PY][PX];  // ring of raw phi planes (zc-2,) zc-1, zc, zc+1 and zc+2 (landing, cp.async)
   double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
-  double ftab[2][64];     // sin / cos force table entries of this block's planes (lz <= 64): the streaming pulls evict
+  double ftab[2][LZ_MAX]; // sin / cos force table entries of this block's planes (lz <= LZ_MAX): the streaming pulls evict
                           // everything from L1, so a per-plane __ldg of the table would wait for L2 every plane
   double ftx[2][TX], fty[2][TY];  // the same for the tile's columns and rows (kept here rather than in 8 registers)
   // FUSED advection (row a8), one plane behind the node update:
@@ -129,8 +137,8 @@ struct GeoTile {
   double acc[NA];         // own slot: phi(t+1) of the previous advected plane, still missing its upper z flux
 };
 
-// Velocity on the seams of the tile columns, written by k_lb_tp<FUSED> and read by k_seam (layouts in accLB_create):
-//   sx[(z ny + y) 2 ntx + 2 bx + s]   u_x at the first (s = 0) / last (s = 1) column of tile column bx
+// Velocity on the seams of the tile columns, written by k_lb_tp<FUSED> and read by k_seam; layouts (carved in accLB_create):
+//   sx[((z ntx + bx) ny + y) 2 + s]   u_x at the first (s = 0) / last (s = 1) column of tile column bx
 //   sy[(z 2 nty + 2 by + s) nx + x]   u_y at the first / last row of tile row by
 //   sz[((2 bz + s) ny + y) nx + x]    u_z at the first / last plane of z chunk bz
 struct Seams {
@@ -139,6 +147,28 @@ struct Seams {
   double* sz;
   int ntx, nty;  // tile columns / rows
 };
+
+// Strip velocity of tile bb along DIR at (x, y, z): first (s = 0) or last (s = 1) cell of the tile.
+template <int DIR>
+__device__ __forceinline__ double seam_vel(const Seams& SM, const Grid& G, int x, int y, int z, int bb, int s) {
+  if (DIR == 0) return __ldg(SM.sx + (((size_t)z * SM.ntx + bb) * G.ny + y) * 2 + s);
+  if (DIR == 1) return __ldg(SM.sy + ((size_t)z * (size_t)(2 * SM.nty) + 2 * bb + s) * G.nx + x);
+  return __ldg(SM.sz + ((size_t)(2 * bb + s) * G.ny + y) * G.nx + x);
+}
+
+// Advective flux (R12) through the seam face in front of the cell with coordinate c0 = first cell of tile
+// b along DIR, at (x, y, z) (whose DIR component is ignored); bp = the tile behind the face.
+template <int DIR>
+__device__ __forceinline__ double seam_face_flux(const Grid& G, const double* __restrict__ phi, const Seams& SM, int x, int y,
+                                                 int z, int c0, int b, int bp) {
+  const size_t plane = (size_t)G.nx * (size_t)G.ny;
+  const int n = DIR == 0 ? G.nx : DIR == 1 ? G.ny : G.nz;
+  const size_t stride = DIR == 0 ? 1 : DIR == 1 ? (size_t)G.nx : plane;
+  const size_t base = (DIR == 2 ? 0 : (size_t)z * plane) + (DIR == 1 ? 0 : (size_t)y * G.nx) + (DIR == 0 ? 0 : x);
+  auto ph = [&](int k) { return __ldg(phi + base + (size_t)wrap_add(c0, k, n) * stride); };
+  return face_flux(seam_vel<DIR>(SM, G, x, y, z, bp, 1), seam_vel<DIR>(SM, G, x, y, z, b, 0), ph(-3), ph(-2), ph(-1), ph(0),
+                   ph(1), ph(2));
+}
 
 // Fused two-phase LB kernel (see the header of this file).  lz = planes per block along z.
 // Iteration zc: phi(zc+1) has landed, fetch phi(zc+2) | derive n, q (tile + 1) and g, |g|, lap (own node, kept in
@@ -297,8 +327,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       *reinterpret_cast<double2*>(d1 + r2) = __ldg(reinterpret_cast<const double2*>(s1 + r2off));
     }
   }
-  double an0 = 0.0, an1 = 0.0, bn0 = 0.0, bn1 = 0.0;  // plane sums of n at planes zc-2, zc-1
-  double aq0 = 0.0, aq1 = 0.0, bq0 = 0.0, bq1 = 0.0;  // plane sums of q
+  // div n and div q at plane z = zc-1 are z combinations of the plane sums a, b (see below) of planes zc-2, zc-1, zc:
+  //   72 div v = a(zc-2) + 4 a(zc-1) + a(zc) + b(zc) - b(zc-2).  Carried per field: P = 4 a(zc-1) + a(zc-2) - b(zc-2) and
+  //   Q = a(zc-1) - b(zc-1), so that 72 div v = P + (a(zc) + b(zc)) and P' = 4 a(zc) + Q, Q' = a(zc) - b(zc).
+  double Pn = 0.0, Qn = 0.0, Pq = 0.0, Qq = 0.0;
   double gp[3] = {0.0, 0.0, 0.0}, gnp = 0.0, lapp = 0.0;  // g, |g|, lap phi of the own node at plane zc-1
   // FUSED: u_z at planes zc-3, zc-2; slot of plane zc-5 in the column history S.col (planes zc-5, zc-4, zc-3)
   double uzm = 0.0, uzc = 0.0;
@@ -318,7 +350,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   int zq2 = pmod(z0 + 1, G.nz);  // wrapped zc + 2, carried (no integer division in the march)
   int sb = 0;                    // element offset of the ring slot of plane zc-1 (slot = it mod NR), carried
   const int zc_last = FUSED ? z1 + 1 : z1;  // FUSED: one more iteration to advect the last plane
-  for (int zc = z0 - 1; zc <= zc_last; ++zc) {
+  // One iteration of the march.  STEADY (FAST only): zc in [z0 + 3, z1 - 1], where every phase is active and no plane is
+  // the first or the last of the chunk -- the same code with the chunk-boundary conditions resolved at compile time.
+  auto iteration = [&](const int zc, auto steady_tag) {
+    constexpr bool STEADY = decltype(steady_tag)::value;
     // ring planes zc-1+k, k = 0..3 (k = NR-1 is plane zc-2 when FUSED), as element offsets from S.raw; sb is carried
     constexpr int PSZ = T::PX * T::PY;
     auto ring = [&](int k) -> double* {
@@ -331,7 +366,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       cp_async_wait_but<1>();
       double* rn = ring(3);  // plane zc+2: its slot held plane zc+2-NR, last read before the previous iteration's
                              // second barrier
-      if (zc < z1) {
+      if (STEADY || zc < z1) {
         const double* src = phi + (size_t)zq2 * plane;
         if (r2 >= 0) cp_async_16(rn + r2, src + r2off);
       }
@@ -341,7 +376,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     __syncthreads();
     // ---- derive n, q (tile + 1 rim) and g, |g|, lap (own node) on plane zc           PAPER.md:L61, L104; R17
     double gc[3] = {0.0, 0.0, 0.0}, gnc = 0.0, lapc = 0.0;
-    if (!FUSED || zc <= z1) {
+    if (STEADY || !FUSED || zc <= z1) {
       const double* rm = ring(0);  // plane zc-1
       const double* rc = ring(1);  // plane zc
       const double* rp = ring(2);  // plane zc+1
@@ -396,7 +431,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
 #ifdef XP_NOADV
     const bool adv = false;
 #else
-    const bool adv = FUSED && pz >= z0;  // block-uniform; pz <= z1 - 1 because zc <= z1 + 1
+    const bool adv = FUSED && (STEADY || pz >= z0);  // block-uniform; pz <= z1 - 1 because zc <= z1 + 1
 #endif
     double Tp = 0.0;                     // phi(t+1) of plane pz, accumulated
     if (FUSED) {
@@ -404,6 +439,11 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const double php = rq[o2];
       if (adv) {
         constexpr int PX = T::PX;
+        if (FAST && tid >= NT - 2 * TY) {  // u_x of plane pz on the two x seams of the tile: 2 TY contiguous strip entries
+          const int e = tid - (NT - 2 * TY);
+          SM.sx[(((unsigned)pz * (unsigned)SM.ntx + blockIdx.x) * (unsigned)G.ny + (unsigned)y0) * 2u + (unsigned)e] =
+              S.ux[(e >> 1) * TX + ((e & 1) ? TX - 1 : 0)];
+        }
         const bool xseam = tx == TX - 1 || x + 1 >= G.nx;  // the face to the right is a seam (or the thread idle)
         const bool yseam = ty == TY - 1 || y + 1 >= G.ny;
         const double* row = rq + (ty + 2) * PX + tx;       // phi(x-2 .. x+3) of the own row
@@ -422,8 +462,8 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         // z face (pz-1, pz): phi(pz-3 .. pz+2) = the column history, then planes zc-2, zc-1, zc of the ring
         const int cj1 = cj == 2 ? 0 : cj + 1, cj2 = cj1 == 2 ? 0 : cj1 + 1;
         double Fz = face_flux(uzm, uzc, S.col[cj][tid], S.col[cj1][tid], S.col[cj2][tid], php, ring(0)[o2], ring(1)[o2]);
-        Fz = pz == z0 ? 0.0 : Fz;
-        if (pz > z0 && active) __stcs(phi_new + (size_t)(pz - 1) * plane + o2off, S.acc[tid] - Fz);  // plane pz-1 is complete
+        if (!STEADY) Fz = pz == z0 ? 0.0 : Fz;
+        if (STEADY || (pz > z0 && active)) __stcs(phi_new + (size_t)(pz - 1) * plane + o2off, S.acc[tid] - Fz);  // plane pz-1 is complete
         Tp = S.e[tid] - (Fx - Fxl) - Fy + Fz;
 #ifdef XP_NOFLUX
 #undef face_flux
@@ -435,7 +475,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     __syncthreads();
     if (adv) {
       Tp += ty == 0 ? 0.0 : S.fy[tid - TX];
-      if (pz == z1 - 1) {  // the face above the chunk's last plane is a seam
+      if (!STEADY && pz == z1 - 1) {  // the face above the chunk's last plane is a seam
         if (active) __stcs(phi_new + (size_t)pz * plane + o2off, Tp);
       } else {
         S.acc[tid] = Tp;
@@ -443,7 +483,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     }
     // ---- plane sums of plane zc at the own node:  a = Dx Sy v_x + Sx Dy v_y,  b = Sx Sy v_z
     double an2 = 0.0, bn2 = 0.0, aq2 = 0.0, bq2 = 0.0;
-    if (!FUSED || zc <= z1) {
+    if (STEADY || !FUSED || zc <= z1) {
       constexpr int NX = T::NX;
       auto plane_sums = [&](int c0_, double& a, double& b) {
         const double* vx = &S.nq[c0_][ty][tx];
@@ -462,8 +502,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     }
     const int z = zc - 1;
     double uz_new = 0.0;
-    if (!(z >= z0 && z < z1 && active)) cp_async_commit();
-    if (z >= z0 && z < z1 && active) {
+    const bool node = STEADY || (z >= z0 && z < z1 && active);
+    if (!node) cp_async_commit();
+    if (node) {
       // a1-a2: the pulled populations have landed in this thread's slots; moments, then refill the slots for plane z+1
       cp_async_wait_but<1>();
       if (fast) mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
@@ -471,13 +512,13 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
       if (fast) {  // every warp has read its 27 values out of the landing zone: refill it for plane z+1
         __syncthreads();
-        if (tx < TY && z + 1 < z1) tma_pull(z + 1);
+        if (tx < TY && (STEADY || z + 1 < z1)) tma_pull(z + 1);
       }
-      if (z + 1 < z1) prefetch_pull(z + 1);
+      if (STEADY || z + 1 < z1) prefetch_pull(z + 1);
       else cp_async_commit();
       // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
-      const double kc = (1.0 / 72.0) * (fma(4.0, an1, an0 + an2) + (bn2 - bn0));
-      const double divq = (1.0 / 72.0) * (fma(4.0, aq1, aq0 + aq2) + (bq2 - bq0));
+      const double kc = (1.0 / 72.0) * (Pn + (an2 + bn2));
+      const double divq = (1.0 / 72.0) * (Pq + (aq2 + bq2));
       const double phi0 = ring(0)[o2];  // plane zc-1 = z
 
       const unsigned k = (unsigned)z * plane + o2off;
@@ -507,18 +548,21 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         S.ux[tid] = u[0];
         S.uy[tid] = u[1];
         uz_new = u[2];
-        // velocities on the seams of this tile column, for k_seam
-#ifndef XP_NOSEAMW
-        // (every strip has fewer elements than the grid has nodes: 32-bit indices)
-        const unsigned ix = ((unsigned)z * (unsigned)G.ny + (unsigned)y) * (unsigned)(2 * SM.ntx) + 2u * blockIdx.x;
-        if (tx == 0) SM.sx[ix] = u[0];
-        if (tx == TX - 1 || x == G.nx - 1) SM.sx[ix + 1] = u[0];
-        const unsigned iy = ((unsigned)z * (unsigned)(2 * SM.nty) + 2u * blockIdx.y) * (unsigned)G.nx + (unsigned)x;
-        if (ty == 0) SM.sy[iy] = u[1];
-        if (ty == TY - 1 || y == G.ny - 1) SM.sy[iy + (unsigned)G.nx] = u[1];
-        if (z == z0) SM.sz[(2u * blockIdx.z) * plane + o2off] = u[2];
-        if (z == z1 - 1) SM.sz[(2u * blockIdx.z + 1u) * plane + o2off] = u[2];
-#endif
+        // velocities on the seams of this tile column (every strip has fewer elements than the grid has nodes: 32-bit
+        // indices).  FAST: u_x goes out one iteration later, 2 TY contiguous values from S.ux by one warp (see the
+        // advection phase); u_y only by the two warps that own the first and the last row.
+        if (!FAST) {
+          const unsigned ix = (((unsigned)z * (unsigned)SM.ntx + blockIdx.x) * (unsigned)G.ny + (unsigned)y) * 2u;
+          if (tx == 0) SM.sx[ix] = u[0];
+          if (tx == TX - 1 || x == G.nx - 1) SM.sx[ix + 1] = u[0];
+        }
+        if (!FAST || ty == 0 || ty == TY - 1) {
+          const unsigned iy = ((unsigned)z * (unsigned)(2 * SM.nty) + 2u * blockIdx.y) * (unsigned)G.nx + (unsigned)x;
+          if (ty == 0) SM.sy[iy] = u[1];
+          if (ty == TY - 1 || y == G.ny - 1) SM.sy[iy + (unsigned)G.nx] = u[1];
+        }
+        if (!STEADY && z == z0) SM.sz[(2u * blockIdx.z) * plane + o2off] = u[2];
+        if (!STEADY && z == z1 - 1) SM.sz[(2u * blockIdx.z + 1u) * plane + o2off] = u[2];
       } else {
         uout[k] = u[0];
         uout[(size_t)G.n + k] = u[1];
@@ -526,12 +570,18 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       }
       collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
     }
-    an0 = an1; an1 = an2; bn0 = bn1; bn1 = bn2;
-    aq0 = aq1; aq1 = aq2; bq0 = bq1; bq1 = bq2;
+    Pn = fma(4.0, an2, Qn); Qn = an2 - bn2;
+    Pq = fma(4.0, aq2, Qq); Qq = aq2 - bq2;
     gp[0] = gc[0]; gp[1] = gc[1]; gp[2] = gc[2]; gnp = gnc; lapp = lapc;
     uzm = uzc; uzc = uz_new;
     sb = sb + PSZ == NR * PSZ ? 0 : sb + PSZ;
+  };
+  int zc = z0 - 1;
+  if (FAST && FUSED) {
+    for (; zc < z0 + 3 && zc <= zc_last; ++zc) iteration(zc, std::false_type{});
+    for (; zc <= z1 - 1; ++zc) iteration(zc, std::true_type{});
   }
+  for (; zc <= zc_last; ++zc) iteration(zc, std::false_type{});
 }
 
 // a8 on the seams of the tile columns of k_lb_tp<FUSED> (R12).  A face is a seam when its two cells
@@ -563,21 +613,17 @@ __global__ void __launch_bounds__(128) k_seam(KP P, const double* __restrict__ p
     const unsigned r = t / (unsigned)G.nx;
     y = (int)(r % (unsigned)G.ny); b = (int)(r / (unsigned)G.ny); z = b * tile;
   }
-  const int c0 = b * tile;  // coordinate along DIR of the cell behind the face
+  const int c0 = b * tile;  // coordinate along DIR of the first cell in front of the face
   const int bp = b == 0 ? ntile - 1 : b - 1, bn = b == ntile - 1 ? 0 : b + 1;
   const size_t stride = DIR == 0 ? 1 : DIR == 1 ? (size_t)G.nx : plane;
   const size_t base = (size_t)z * plane + (size_t)y * G.nx + x - (size_t)c0 * stride;  // cell with coordinate 0 along DIR
-  auto ph = [&](int k) { return __ldg(phi + base + (size_t)wrap_add(c0, k, n) * stride); };
-  auto vel = [&](int bb, int s) {  // strip velocity of tile bb, first (s = 0) or last (s = 1) cell along DIR
-    if (DIR == 0) return __ldg(SM.sx + ((size_t)z * G.ny + y) * (size_t)(2 * SM.ntx) + 2 * bb + s);
-    if (DIR == 1) return __ldg(SM.sy + ((size_t)z * (size_t)(2 * SM.nty) + 2 * bb + s) * G.nx + x);
-    return __ldg(SM.sz + (size_t)(2 * bb + s) * plane + (size_t)y * G.nx + x);
-  };
-  const double p_3 = ph(-3), p_2 = ph(-2), p_1 = ph(-1), p0 = ph(0), p1 = ph(1), p2 = ph(2);
-  const double uLs = vel(bp, 1), uRs = vel(b, 0);
-  const double F = face_flux(uLs, uRs, p_3, p_2, p_1, p0, p1, p2);
+  const double F = seam_face_flux<DIR>(G, phi, SM, x, y, z, c0, b, bp);
   double dR = F;
-  if (min(tile, n - c0) == 1) dR -= face_flux(vel(b, 1), vel(bn, 0), p_2, p_1, p0, p1, p2, ph(3));  // one-cell tile: its upper face too
+  if (min(tile, n - c0) == 1) {  // one-cell tile: its upper face too
+    auto ph = [&](int k) { return __ldg(phi + base + (size_t)wrap_add(c0, k, n) * stride); };
+    dR -= face_flux(seam_vel<DIR>(SM, G, x, y, z, b, 1), seam_vel<DIR>(SM, G, x, y, z, bn, 0), ph(-2), ph(-1), ph(0), ph(1),
+                    ph(2), ph(3));
+  }
   double* const cR = phi_new + base + (size_t)c0 * stride;
   *cR = *cR + dR;
   if (min(tile, n - bp * tile) > 1) {
