@@ -121,7 +121,7 @@ struct GeoTile {
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
   static constexpr int NR = FUSED ? 5 : 4;
   alignas(16) double raw[NR][PY][PX];  // ring of raw phi planes (zc-2,) zc-1, zc, zc+1 and zc+2 (landing, cp.async)
-  double nq[6][NY][NX];   // n_x n_y n_z q_x q_y q_z of plane zc, q = phi (1 - phi) n
+  alignas(16) double2 nq[3][NY][NX];  // (n_c, q_c), c = x, y, z, of plane zc, q = phi (1 - phi) n: one 16-byte access serves both
   double ftab[2][LZ_MAX]; // sin / cos force table entries of this block's planes (lz <= LZ_MAX): the streaming pulls evict
                           // everything from L1, so a per-plane __ldg of the table would wait for L2 every plane
   double ftx[2][TX], fty[2][TY];  // the same for the tile's columns and rows (kept here rather than in 8 registers)
@@ -129,7 +129,8 @@ struct GeoTile {
   static constexpr int NA = FUSED ? TX * TY : 1;
   double ux[NA], uy[NA];  // u_x, u_y of the plane updated last (read by the neighbour lane / row)
   double fy[NA];          // flux through the y face above the node
-  double e[NA];           // own slot: phi + r of the plane updated last
+  double e[FUSED ? 3 : 1][NA];  // own slots: phi + D lap phi (written when the plane is derived) - kappa div q (added at its
+                                // node update) of planes zc-2, zc-1, zc; slot = plane mod 3 (as col)
   double col[3][NA];      // own slots: phi of the three planes older than the ring (z-face window)
 #ifdef XP_PAD
   double pad_[XP_PAD];
@@ -406,17 +407,15 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const double inv = div_pos(1.0, gn + 1e-12);
         const double pq = ph * (1.0 - ph);
         const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
-        S.nq[0][j][i] = nx_;
-        S.nq[1][j][i] = ny_;
-        S.nq[2][j][i] = nz_;
-        S.nq[3][j][i] = pq * nx_;
-        S.nq[4][j][i] = pq * ny_;
-        S.nq[5][j][i] = pq * nz_;
+        S.nq[0][j][i] = make_double2(nx_, pq * nx_);
+        S.nq[1][j][i] = make_double2(ny_, pq * ny_);
+        S.nq[2][j][i] = make_double2(nz_, pq * nz_);
         if (own_node) {
           const double s0 = fma(4.0, t01, t00 + t02), s1 = fma(4.0, t11, t10 + t12), s2 = fma(4.0, t21, t20 + t22);
           gc[0] = gx; gc[1] = gy; gc[2] = gz;
           gnc = gn;
           lapc = 6.0 * (fma(4.0, s1, s0 + s2) * (1.0 / 216.0) - ph);  // R7
+          if (FUSED) S.e[cj >= 1 ? cj - 1 : 2][tid] = fma(P.D, lapc, ph);  // slot of plane zc = (cj + 2) mod 3
         }
       };
       derive(ty + 1, tx + 1, true);
@@ -464,13 +463,26 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         double Fz = face_flux(uzm, uzc, S.col[cj][tid], S.col[cj1][tid], S.col[cj2][tid], php, ring(0)[o2], ring(1)[o2]);
         if (!STEADY) Fz = pz == z0 ? 0.0 : Fz;
         if (STEADY || (pz > z0 && active)) __stcs(phi_new + (size_t)(pz - 1) * plane + o2off, S.acc[tid] - Fz);  // plane pz-1 is complete
-        Tp = S.e[tid] - (Fx - Fxl) - Fy + Fz;
+        Tp = S.e[cj][tid] - (Fx - Fxl) - Fy + Fz;
 #ifdef XP_NOFLUX
 #undef face_flux
 #endif
       }
       S.col[cj][tid] = php;  // plane zc-2 replaces plane zc-5
       cj = cj == 2 ? 0 : cj + 1;
+    }
+    // ---- a1-a2 of plane z = zc - 1: the pulled populations have landed in this thread's slots; moments.  Done before the
+    // barrier so that ONE barrier both publishes n, q, the y fluxes and hands the landing zone over for the next pull.
+    const int z = zc - 1;
+    const bool node = STEADY || (z >= z0 && z < z1 && active);
+    Moments M;
+    if (node) {
+      cp_async_wait_but<1>();
+      if (fast) {
+        __syncwarp();  // the edge elements were copied by other lanes of this warp
+        mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
+      }
+      moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
     }
     __syncthreads();
     if (adv) {
@@ -485,35 +497,28 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     double an2 = 0.0, bn2 = 0.0, aq2 = 0.0, bq2 = 0.0;
     if (STEADY || !FUSED || zc <= z1) {
       constexpr int NX = T::NX;
-      auto plane_sums = [&](int c0_, double& a, double& b) {
-        const double* vx = &S.nq[c0_][ty][tx];
-        const double* vy = &S.nq[c0_ + 1][ty][tx];
-        const double* vz = &S.nq[c0_ + 2][ty][tx];
-        const double ax = fma(4.0, vx[NX + 2] - vx[NX], (vx[2] - vx[0]) + (vx[2 * NX + 2] - vx[2 * NX]));
-        const double ay = fma(4.0, vy[2 * NX + 1] - vy[1], (vy[2 * NX] - vy[0]) + (vy[2 * NX + 2] - vy[2]));
-        a = ax + ay;
-        const double r0 = fma(4.0, vz[1], vz[0] + vz[2]);
-        const double r1 = fma(4.0, vz[NX + 1], vz[NX] + vz[NX + 2]);
-        const double r2_ = fma(4.0, vz[2 * NX + 1], vz[2 * NX] + vz[2 * NX + 2]);
-        b = fma(4.0, r1, r0 + r2_);
-      };
-      plane_sums(0, an2, bn2);
-      plane_sums(3, aq2, bq2);
+      // (n and q together: every shared-memory access fetches the pair (n_c, q_c))
+      const double2* vx = &S.nq[0][ty][tx];
+      const double2* vy = &S.nq[1][ty][tx];
+      const double2* vz = &S.nq[2][ty][tx];
+      const double2 x00 = vx[0], x02 = vx[2], x10 = vx[NX], x12 = vx[NX + 2], x20 = vx[2 * NX], x22 = vx[2 * NX + 2];
+      const double2 y00 = vy[0], y01 = vy[1], y02 = vy[2], y20 = vy[2 * NX], y21 = vy[2 * NX + 1], y22 = vy[2 * NX + 2];
+      const double axn = fma(4.0, x12.x - x10.x, (x02.x - x00.x) + (x22.x - x20.x));
+      const double axq = fma(4.0, x12.y - x10.y, (x02.y - x00.y) + (x22.y - x20.y));
+      const double ayn = fma(4.0, y21.x - y01.x, (y20.x - y00.x) + (y22.x - y02.x));
+      const double ayq = fma(4.0, y21.y - y01.y, (y20.y - y00.y) + (y22.y - y02.y));
+      an2 = axn + ayn;
+      aq2 = axq + ayq;
+      const double2 z00 = vz[0], z01 = vz[1], z02 = vz[2], z10 = vz[NX], z11 = vz[NX + 1], z12 = vz[NX + 2];
+      const double2 z20 = vz[2 * NX], z21 = vz[2 * NX + 1], z22 = vz[2 * NX + 2];
+      bn2 = fma(4.0, fma(4.0, z11.x, z10.x + z12.x), fma(4.0, z01.x, z00.x + z02.x) + fma(4.0, z21.x, z20.x + z22.x));
+      bq2 = fma(4.0, fma(4.0, z11.y, z10.y + z12.y), fma(4.0, z01.y, z00.y + z02.y) + fma(4.0, z21.y, z20.y + z22.y));
     }
-    const int z = zc - 1;
     double uz_new = 0.0;
-    const bool node = STEADY || (z >= z0 && z < z1 && active);
     if (!node) cp_async_commit();
     if (node) {
-      // a1-a2: the pulled populations have landed in this thread's slots; moments, then refill the slots for plane z+1
-      cp_async_wait_but<1>();
-      if (fast) mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
-      Moments M;
-      moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
-      if (fast) {  // every warp has read its 27 values out of the landing zone: refill it for plane z+1
-        __syncthreads();
-        if (tx < TY && (STEADY || z + 1 < z1)) tma_pull(z + 1);
-      }
+      // every warp has read its 27 values out of the landing zone (barrier above): refill it for plane z+1
+      if (fast && (STEADY || z + 1 < z1) && tx < TY) tma_pull(z + 1);
       if (STEADY || z + 1 < z1) prefetch_pull(z + 1);
       else cp_async_commit();
       // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
@@ -522,9 +527,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const double phi0 = ring(0)[o2];  // plane zc-1 = z
 
       const unsigned k = (unsigned)z * plane + o2off;
-      const double rr = P.D * lapp - P.kappa * divq;  // phi-only part of Eq. 3
-      if (FUSED) S.e[tid] = phi0 + rr;
-      else rout[k] = rr;
+      // phi-only part of Eq. 3: r = D lap phi - kappa div q
+      if (FUSED) S.e[cj][tid] -= P.kappa * divq;  // (cj was advanced above: slot of plane z = zc-1)
+      else rout[k] = P.D * lapp - P.kappa * divq;
 
       // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
       double Fb[3] = {0.0, 0.0, 0.0};
