@@ -269,36 +269,40 @@ def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=T
     return out
 
 
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of a kernel at 512^3, from the `ncu --set full`
+# captures whose summaries are committed under profiles/ (bench.py does not read that folder).  A capture describes the
+# kernel as it was at the commit named; when a kernel changes, its entry is re-measured or removed (then `traffic` is null).
+NCU_TRAFFIC = {
+}
+
+
 def roofline_of(meas, steps, fp32):
-    """Roofline object for the dominant kernel, from its CUDA-event durations inside the timed region.  The dominant
-    kernel is k_step_tp (the whole two-phase step as one persistent kernel: algorithmic bytes = 54 populations + phi
-    read + phi written per node) or k_lb (the fused LB step: 54 populations per node)."""
+    """Roofline object.  `achieved`/`frac` are for the WHOLE step (the north-star's figure of merit): algorithmic bytes of a
+    step (54 populations, + phi read + phi written when two-phase) x nodes / the CUDA-event time of the timed region.  The
+    dominant kernel (largest summed CUDA-event time inside the timed region; events bracket every launch on the launching
+    stream) is reported beside it with its own algorithmic bytes: the fused two-phase kernel k_lb_tp moves all of the
+    step's algorithmic bytes (the seam kernels only patch phi), the single-phase k_lb the 54 populations."""
     n3 = meas["n"] ** 3
     kernels = {k: v for k, v in meas["kernels"].items() if v[1]}
     name = max(kernels, key=lambda k: kernels[k][0])
     ms_k, cnt_k = kernels[name]
-    bpl = step_bytes_per_lup(fp32, meas["two_phase"]) if name == "k_step_tp" else lb_bytes_per_lup(fp32)
+    step_bpl = step_bytes_per_lup(fp32, meas["two_phase"])
+    bpl = step_bpl if name == "k_lb_tp" and "k_advect" not in kernels else lb_bytes_per_lup(fp32)
     peak, how = hbm_peak()
     per_launch_ms = ms_k / max(cnt_k, 1)
-    achieved = bpl * n3 / (per_launch_ms * 1e-3) / 1e9
+    k_achieved = bpl * n3 / (per_launch_ms * 1e-3) / 1e9
     total_ms = sum(v[0] for v in kernels.values())
-    r = {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": peak, "peak_source": how, "unit": "GB/s",
-         "frac": achieved / peak, "traffic": None, "bytes_per_launch": bpl * n3, "bytes_per_lup": bpl,
-         "kernel_ms_per_launch": per_launch_ms, "kernel_share_of_step": ms_k / total_ms if total_ms else None,
-         "kernels_ms_per_step": {k: v[0] / steps for k, v in kernels.items()},
-         "step_bytes_per_lup": step_bytes_per_lup(fp32, meas["two_phase"])}
-    r["step_achieved"] = r["step_bytes_per_lup"] * n3 * steps / (meas["ms"] * 1e-3) / 1e9
-    r["step_frac"] = r["step_achieved"] / peak
-    t = ROOT / "profiles" / "r01_traffic.csv"  # dram bytes per launch of the kernel from the committed ncu --set full capture
-    try:
-        key = f"{name}_{'two' if meas['two_phase'] else 'single'}_{'fp32' if fp32 else 'fp64'}_{meas['n']}"
-        for line in t.read_text().splitlines()[1:]:
-            k, v = line.split(",")
-            if k == key:
-                r["traffic"] = int(v)
-    except Exception:
-        pass
-    return r
+    achieved = step_bpl * n3 * steps / (meas["ms"] * 1e-3) / 1e9
+    key = (name, "two" if meas["two_phase"] else "single", "fp32" if fp32 else "fp64", meas["n"])
+    traffic, source = NCU_TRAFFIC.get(key, (None, None))
+    return {"bound": "hbm", "scope": "whole step (all kernels of the timed region)", "achieved": achieved, "peak": peak,
+            "peak_source": how, "unit": "GB/s", "frac": achieved / peak, "bytes_per_lup": step_bpl,
+            "bytes_per_step": step_bpl * n3, "traffic": traffic, "traffic_source": source, "traffic_kernel": name,
+            "kernel": name, "kernel_bytes_per_lup": bpl, "kernel_bytes_per_launch": bpl * n3,
+            "kernel_ms_per_launch": per_launch_ms, "kernel_achieved": k_achieved, "kernel_frac": k_achieved / peak,
+            "kernel_share_of_step": ms_k / total_ms if total_ms else None,
+            "kernels_ms_per_step": {k: v[0] / steps for k, v in kernels.items()},
+            "step_achieved": achieved, "step_frac": achieved / peak, "step_bytes_per_lup": step_bpl}
 
 
 def max_over_ranks(values, device=None):
@@ -373,6 +377,15 @@ def run_cuda(args):
                        "wall_ms_per_call": e["wall_ms"],
                        "call": f"accLB_run_host(nsteps={args.steps}): pinned host p*,u,phi -> init -> steps -> moments + "
                                "diagnostics -> pinned host"}
+    if world == 1 and two_phase and not args.no_single:
+        # the other half of the north-star bar: the fused single-phase step (config-2 set-up at the same size), timed in
+        # this process with the same steps / warm-up
+        sp_cfg = make_workload("hit", args.n)
+        sp = measure_cuda(sp_cfg, args.steps, args.warmup, local_rank=local_rank, fp32=bool(args.fp32), e2e=False)
+        line["single_phase"] = {"workload": f"hit {args.n}^3 single-phase; " + WORKLOADS["hit"][1],
+                                "value": n3 * args.steps / (sp["ms"] * 1e-3) / 1e9, "unit": UNIT,
+                                "ms_per_step": sp["ms"] / args.steps, "gpu_launches": sp["launches"], "clocks": sp["clocks"],
+                                "roofline": roofline_of(sp, args.steps, bool(args.fp32))}
     if world == 1 and not args.no_cpu:
         import oracle
 
@@ -424,6 +437,7 @@ def main():
     ap.add_argument("--variant", type=int, default=None, help="kernel variant (accLB_set_variant), default = best")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-single", action="store_true", help="skip the single_phase leg of a two-phase run")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--sweep-sizes", default="64,128,256,384,512")
     ap.add_argument("--sweep-out", default=None)

@@ -95,7 +95,7 @@ def workspace_bytes(nx, ny, nz, params):
 class AccLB:
     """One periodic box on one GPU.  Fields are fp64 CUDA tensors: scalars [nz][ny][nx], vectors [3][nz][ny][nx]."""
 
-    def __init__(self, nx, ny, nz, *, device=0, stream=None, **params):
+    def __init__(self, nx, ny, nz, *, device=0, stream=None, workspace=None, **params):
         import torch
 
         L = load()
@@ -112,7 +112,10 @@ class AccLB:
         nbytes = L.accLB_workspace_bytes(nx, ny, nz, C.byref(self.params))
         if nbytes == 0:
             raise AccLBError(-1, f"invalid grid {nx}x{ny}x{nz} or parameters")
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)  # torch owns device memory
+        if workspace is None:
+            workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)  # torch owns device memory
+        assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous() and workspace.numel() >= nbytes
+        self.workspace = workspace  # (a caller-provided block, e.g. a view into a larger tensor, is used as it is)
         self.workspace_bytes = nbytes
         h = C.c_void_p()
         _check(L.accLB_create(C.byref(h), nx, ny, nz, C.byref(self.params), self.workspace.data_ptr(), nbytes))

@@ -472,8 +472,46 @@ struct accLB_ctx {
   int variant;
   int profiling;
   struct Rec { int kind; cudaEvent_t e0, e1; };
-  std::vector<Rec> recs;
+  std::vector<Rec> recs;                 // at most REC_MAX pending event pairs; older ones are folded into the totals
+  double folded_ms[ACCLB_NKERNELS];
+  long long folded_count[ACCLB_NKERNELS];
 };
+
+// Selects the context's device for the duration of an ABI call and restores the caller's current device afterwards
+// (a multi-GPU process keeps its own current device; "replicas only").
+struct DeviceGuard {
+  int prev = -1;
+  bool ok;
+  explicit DeviceGuard(int dev) {
+    ok = cudaGetDevice(&prev) == cudaSuccess;
+    if (ok && prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+    else if (ok) prev = -1;  // nothing to restore
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+#define GUARD_DEVICE(s_)                                                                          \
+  DeviceGuard guard_((s_)->prm.device);                                                            \
+  if (!guard_.ok) return fail(ACCLB_ECUDA, "cannot select device %d", (s_)->prm.device)
+
+constexpr size_t REC_MAX = 4096;
+// Waits for the pending event pairs and adds their durations to the per-kernel totals (bounded host memory however long
+// profiling stays on).
+static void fold_records(accLB_ctx* s) {
+  if (s->recs.empty()) return;
+  cudaEventSynchronize(s->recs.back().e1);
+  for (auto& r : s->recs) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, r.e0, r.e1) == cudaSuccess && r.kind >= 0 && r.kind < ACCLB_NKERNELS) {
+      s->folded_ms[r.kind] += (double)t;
+      s->folded_count[r.kind] += 1;
+    }
+    cudaEventDestroy(r.e0);
+    cudaEventDestroy(r.e1);
+  }
+  s->recs.clear();
+}
 
 // Counts a kernel launch and, when profiling is on, brackets it with two events on the context's stream.
 struct LaunchScope {
@@ -492,6 +530,7 @@ struct LaunchScope {
     if (on) {
       cudaEventRecord(r.e1, s->stream);
       s->recs.push_back(r);
+      if (s->recs.size() >= REC_MAX) fold_records(s);
     }
   }
 };
@@ -689,7 +728,8 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   int ndev = 0;
   CK(cudaGetDeviceCount(&ndev));
   if (p->device < 0 || p->device >= ndev) return fail(ACCLB_EINVAL, "accLB_create: device %d of %d", p->device, ndev);
-  CK(cudaSetDevice(p->device));
+  DeviceGuard guard_(p->device);
+  if (!guard_.ok) return fail(ACCLB_ECUDA, "accLB_create: cannot select device %d", p->device);
 
   accLB_ctx* s = new (std::nothrow) accLB_ctx();
   if (!s) return fail(ACCLB_EINVAL, "accLB_create: out of host memory");
@@ -715,6 +755,7 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   s->lz = planes_per_block(nx, ny, nz, LBT_TX, LBT_TY);
   s->stage = p->host_staging ? (double*)w : nullptr; w += c.stage;
   s->cur = 0; s->step = 0; s->launches = 0; s->variant = 0; s->profiling = 0;
+  for (int k = 0; k < ACCLB_NKERNELS; ++k) { s->folded_ms[k] = 0.0; s->folded_count[k] = 0; }
 
   KP& k = s->kp;
   k.G.nx = nx; k.G.ny = ny; k.G.nz = nz; k.G.n = (unsigned)s->n;
@@ -767,7 +808,7 @@ static int launch_normal(accLB_ctx* s) {
 int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* phi) {
   if (!s || !rho || !u) return fail(ACCLB_EINVAL, "accLB_init: NULL argument");
   if (s->prm.two_phase && !phi) return fail(ACCLB_EINVAL, "accLB_init: phi is NULL for a two-phase context");
-  CK(cudaSetDevice(s->prm.device));
+  GUARD_DEVICE(s);
   s->cur = 0;
   s->step = 0;
   const unsigned nb = blocks_for(s->n, 128);
@@ -793,7 +834,7 @@ int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* p
 
 int accLB_step(accLB_ctx* s, int nsteps) {
   if (!s || nsteps < 0) return fail(ACCLB_EINVAL, "accLB_step: NULL context or negative nsteps");
-  CK(cudaSetDevice(s->prm.device));
+  GUARD_DEVICE(s);
   const unsigned nb = blocks_for(s->n, 128);
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
@@ -840,7 +881,7 @@ int accLB_step(accLB_ctx* s, int nsteps) {
 
 int accLB_moments(accLB_ctx* s, double* rho, double* u, double* phi) {
   if (!s) return fail(ACCLB_EINVAL, "accLB_moments: NULL context");
-  CK(cudaSetDevice(s->prm.device));
+  GUARD_DEVICE(s);
   const unsigned nb = blocks_for(s->n, 128);
   const int c = s->cur;
   if (s->prm.two_phase) {
@@ -867,7 +908,7 @@ int accLB_moments(accLB_ctx* s, double* rho, double* u, double* phi) {
 
 int accLB_diagnostics(accLB_ctx* s, double* out, int n_out) {
   if (!s || !out || n_out < ACCLB_NDIAG) return fail(ACCLB_EINVAL, "accLB_diagnostics: NULL argument or n_out < %d", ACCLB_NDIAG);
-  CK(cudaSetDevice(s->prm.device));
+  GUARD_DEVICE(s);
   const int c = s->cur;
   CK(cudaMemsetAsync(s->acc, 0, 16 * 8, s->stream));
   unsigned nb = blocks_for(s->n, DIAG_THREADS);
@@ -912,7 +953,7 @@ int accLB_run_host(accLB_ctx* s, const double* h_rho, const double* h_u, const d
   if (!s || !h_rho || !h_u || nsteps < 0) return fail(ACCLB_EINVAL, "accLB_run_host: NULL argument or negative nsteps");
   if (!s->stage) return fail(ACCLB_EINVAL, "accLB_run_host: context was created without host_staging");
   if (s->prm.two_phase && !h_phi) return fail(ACCLB_EINVAL, "accLB_run_host: h_phi is NULL for a two-phase context");
-  CK(cudaSetDevice(s->prm.device));
+  GUARD_DEVICE(s);
   const size_t n = s->n;
   double* d_rho = s->stage;
   double* d_u = s->stage + n;
@@ -964,17 +1005,15 @@ int accLB_profile(accLB_ctx* s, int enable) {
 
 int accLB_profile_read(accLB_ctx* s, double* ms, long long* count, int n) {
   if (!s || !ms || !count || n < 1) return fail(ACCLB_EINVAL, "accLB_profile_read: NULL argument");
-  CK(cudaSetDevice(s->prm.device));
+  GUARD_DEVICE(s);
   CK(cudaStreamSynchronize(s->stream));
-  for (auto& r : s->recs) {
-    float t = 0.f;
-    CK(cudaEventElapsedTime(&t, r.e0, r.e1));
-    if (r.kind < n && r.kind < ACCLB_NKERNELS) {
-      ms[r.kind] += (double)t;
-      count[r.kind] += 1;
-    }
+  fold_records(s);
+  for (int k = 0; k < n && k < ACCLB_NKERNELS; ++k) {
+    ms[k] += s->folded_ms[k];
+    count[k] += s->folded_count[k];
+    s->folded_ms[k] = 0.0;
+    s->folded_count[k] = 0;
   }
-  drop_records(s);
   return ACCLB_OK;
 }
 

@@ -35,9 +35,23 @@ def tgv_fields(n=32, u0=0.02):
     return rho, u
 
 
+_VELOCITY_CACHE = {}
+
+
 def hit_velocity(n, urms=0.03, seed=SEED_VELOCITY, k_peak=4.0):
     """Configs 2/4/5: seeded random solenoidal field with shell spectrum E(k) ~ k^4 exp(-2 (k/k_peak)^2),
-    normalised to sqrt(<u.u>/3) = urms (R28)."""
+    normalised to sqrt(<u.u>/3) = urms (R28).  The last field is kept (read-only): configs 2 and 4 of one size share it."""
+    key = (n, urms, seed, k_peak)
+    if key in _VELOCITY_CACHE:
+        return _VELOCITY_CACHE[key]
+    _VELOCITY_CACHE.clear()
+    u = _hit_velocity(n, urms, seed, k_peak)
+    u.setflags(write=False)
+    _VELOCITY_CACHE[key] = u
+    return u
+
+
+def _hit_velocity(n, urms, seed, k_peak):
     rng = np.random.Generator(np.random.PCG64(seed))
     a = rng.standard_normal((3, n, n, n))
     ah = _fft.rfftn(a, axes=(1, 2, 3), **_FFT_KW)
