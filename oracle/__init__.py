@@ -39,6 +39,7 @@ class OracleParams(C.Structure):
         ("mobility", C.c_double), ("width", C.c_double),
         ("force_type", C.c_int), ("force_amp", C.c_double), ("force_k", C.c_int),
         ("force_period", C.c_int * 3), ("force_origin", C.c_int * 3),
+        ("gravity", C.c_double * 3), ("rho_ref", C.c_double), ("phi_rk3", C.c_int),
     ]
 
 
@@ -93,10 +94,11 @@ class Oracle:
 
     def __init__(self, nx, ny, nz, *, tau, two_phase=False, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0,
                  width=4.0, force_type=0, force_amp=0.0, force_k=1, force_period=(0, 0, 0),
-                 force_origin=(0, 0, 0)):
+                 force_origin=(0, 0, 0), gravity=(0.0, 0.0, 0.0), rho_ref=0.0, phi_rk3=0):
         self.params = OracleParams(nx, ny, nz, tau, int(two_phase), rho_l, rho_g, sigma, mobility, width,
                                    force_type, force_amp, force_k,
-                                   (C.c_int * 3)(*force_period), (C.c_int * 3)(*force_origin))
+                                   (C.c_int * 3)(*force_period), (C.c_int * 3)(*force_origin),
+                                   (C.c_double * 3)(*gravity), rho_ref, int(phi_rk3))
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
         self.two_phase = bool(two_phase)

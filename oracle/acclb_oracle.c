@@ -17,7 +17,8 @@
  * (x+c+N)%N periodic wraps.  Build with -ffp-contract=off so the arithmetic is what is written.
  *
  * Parity-unpinned parts (the paper fixes nothing to pin them against):
- *   - WENO5 variant / epsilon (R12), forward-Euler phi integrator (R13), step ordering (R14).
+ *   - WENO5 variant / epsilon (R12), the choice of phi integrator (R13 forward Euler, R32 SSP-RK3: both pinned as
+ *     schemes, the paper names neither), step ordering (R14), the reference density of the buoyancy force (R31).
  *   Pinned since round 2 (tests/test_oracle_physics.py): direction, upwind side and order of the phi advection
  *   (face_flux / pass_allen_cahn), and F^nu (R9) on a prescribed shear against nu (du + du^T).grad rho.
  */
@@ -44,6 +45,9 @@ typedef struct {
   int force_k;         /* forcing wavenumber in units of 2 pi / L */
   int force_period[3]; /* box the forcing is periodic on (0 -> nx,ny,nz); lets a sub-box of a larger */
   int force_origin[3]; /* problem be evaluated: global coordinate of local node (0,0,0)              */
+  double gravity[3];   /* buoyancy F^g = (rho(phi) - rho_ref) g   PAPER.md:L193, L203 ("buoyant gas phase"); R31 */
+  double rho_ref;      /* reference density of the buoyancy force (the harness sets the mean density: no net force) */
+  int phi_rk3;         /* 0: forward Euler (R13) | 1: SSP-RK3 for phi within one LB step   PAPER.md:L110; R32 */
 } oracle_params;
 
 typedef struct {
@@ -59,6 +63,7 @@ typedef struct {
   double *m;            /* [3][n]  raw first moment sum_i f_i c_i (for diagnostics)           */
   double *g;            /* [3][n]  grad phi                                                   */
   double *nrm;          /* [3][n]  interface normal                                           */
+  double *phi_s, *nrm_s; /* RK3 only: stage field and its normal                              */
 } oracle_state;
 
 static int C[Q][3];
@@ -170,11 +175,10 @@ static double weno5(double a, double b, double c, double d, double e) {
 
 /* Advective flux of phi through the face between x and x+e along axis ax (R12: flux form, face velocity =
  * arithmetic mean, upwinding by its sign). */
-static double face_flux(const oracle_state *s, int ax, int x, int y, int z) {
+static double face_flux(const oracle_state *s, const double *ph, int ax, int x, int y, int z) {
   int e[3] = {0, 0, 0};
   e[ax] = 1;
   const double *ue = s->u + (size_t)ax * s->n;
-  const double *ph = s->phi;
 #define PH(k) ph[at(s, x + (k)*e[0], y + (k)*e[1], z + (k)*e[2])]
   double uf = 0.5 * (ue[at(s, x, y, z)] + ue[at(s, x + e[0], y + e[1], z + e[2])]);
   double pf;
@@ -187,7 +191,7 @@ static double face_flux(const oracle_state *s, int ax, int x, int y, int z) {
 }
 
 /* ---- O2 (first half): g = grad phi, n = g / (|g| + 1e-12) for every node   PAPER.md:L61, L104; R17 ---- */
-static void pass_geometry(oracle_state *s) {
+static void geometry_of(const oracle_state *s, const double *phi, double *g_out /* may be NULL */, double *nrm_out) {
   const int nx = s->p.nx, ny = s->p.ny, nz = s->p.nz;
   const size_t n = s->n;
 #pragma omp parallel for collapse(2) schedule(static)
@@ -196,14 +200,15 @@ static void pass_geometry(oracle_state *s) {
       for (int x = 0; x < nx; ++x) {
         size_t k = at(s, x, y, z);
         double g[3];
-        grad_at(s, s->phi, x, y, z, g);
+        grad_at(s, phi, x, y, z, g);
         double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
         for (int al = 0; al < 3; ++al) {
-          s->g[al * n + k] = g[al];
-          s->nrm[al * n + k] = g[al] / (gn + 1e-12);
+          if (g_out) g_out[al * n + k] = g[al];
+          nrm_out[al * n + k] = g[al] / (gn + 1e-12);
         }
       }
 }
+static void pass_geometry(oracle_state *s) { geometry_of(s, s->phi, s->g, s->nrm); }
 
 /* Total force at a node from phi-geometry and the node's own moments (O2 second half + O3).
  * with_visc = 0 drops F^nu (used by init, R15).  Returns F in F[3] and rho. */
@@ -212,8 +217,8 @@ static double total_force(const oracle_state *s, int x, int y, int z, double pst
   const oracle_params *p = &s->p;
   double Fb[3];
   body_force(p, x, y, z, Fb);
-  if (!p->two_phase) { /* single component: rho == 1, F = F^b */
-    for (int al = 0; al < 3; ++al) F[al] = Fb[al];
+  if (!p->two_phase) { /* single component: rho == 1, F = F^b (+ the uniform (1 - rho_ref) g, R31) */
+    for (int al = 0; al < 3; ++al) F[al] = Fb[al] + (1.0 - p->rho_ref) * p->gravity[al];
     return 1.0;
   }
   const size_t n = s->n, k = at(s, x, y, z);
@@ -227,15 +232,16 @@ static double total_force(const oracle_state *s, int x, int y, int z, double pst
   }
   kc /= CS2;
   double rho = p->rho_g + (p->rho_l - p->rho_g) * s->phi[k]; /* PAPER.md:L102 */
-  double drho[3], Fs[3], Fp[3], Fv[3] = {0.0, 0.0, 0.0};
+  double drho[3], Fs[3], Fp[3], Fg[3], Fv[3] = {0.0, 0.0, 0.0};
   for (int al = 0; al < 3; ++al) {
+    Fg[al] = (rho - p->rho_ref) * p->gravity[al]; /* buoyancy, PAPER.md:L193, L203; R31 */
     drho[al] = (p->rho_l - p->rho_g) * g[al];
     Fs[al] = -p->sigma * (1.5 * p->width) * kc * gn * g[al]; /* PAPER.md:L102 + normalisation R8 */
     Fp[al] = -pstar * CS2 * drho[al];                        /* PAPER.md:L102 */
   }
   if (with_visc && p->rho_l != p->rho_g) { /* PAPER.md:L104 read as R9 */
     double ut[3];
-    for (int al = 0; al < 3; ++al) ut[al] = m[al] + (Fs[al] + Fp[al] + Fb[al]) / (2.0 * rho);
+    for (int al = 0; al < 3; ++al) ut[al] = m[al] + (Fs[al] + Fp[al] + Fb[al] + Fg[al]) / (2.0 * rho);
     double pref = (p->tau - 0.5) / p->tau; /* nu omega / cs2 */
     for (int al = 0; al < 3; ++al) {
       double acc = 0.0;
@@ -244,7 +250,7 @@ static double total_force(const oracle_state *s, int x, int y, int z, double pst
       Fv[al] = -pref * acc;
     }
   }
-  for (int al = 0; al < 3; ++al) F[al] = Fs[al] + Fp[al] + Fv[al] + Fb[al]; /* Eq. 8, PAPER.md:L100 (+ F^b) */
+  for (int al = 0; al < 3; ++al) F[al] = Fs[al] + Fp[al] + Fv[al] + Fb[al] + Fg[al]; /* Eq. 8, PAPER.md:L100 (+ F^b, F^g) */
   return rho;
 }
 
@@ -313,9 +319,12 @@ static void pass_reconstruct_stream(oracle_state *s) {
       }
 }
 
-/* ---- pass 3: O8 conservative Allen-Cahn, forward Euler (R13), flux-form WENO5 advection (R12), lattice
- * Laplacian (R7) and lattice divergence of the sharpening flux phi(1-phi)n   PAPER.md:L61 (Eq. 3), L67, L104 ---- */
-static void pass_allen_cahn(oracle_state *s) {
+/* ---- pass 3: O8 conservative Allen-Cahn, flux-form WENO5 advection (R12), lattice Laplacian (R7) and lattice divergence
+ * of the sharpening flux phi(1-phi)n   PAPER.md:L61 (Eq. 3), L67, L104.
+ * One evaluation: out = a * base + b * (phi + L(phi)),  L(phi) = -div(u phi) + D lap phi - kappa div(phi (1 - phi) n),
+ * with n = n(phi) given in nrm and u = u(t) of pass 1.  Forward Euler (R13) is a = 0, b = 1. ---- */
+static void allen_cahn_stage(const oracle_state *s, const double *phi, const double *nrm, const double *base, double a,
+                             double b, double *out) {
   const int nx = s->p.nx, ny = s->p.ny, nz = s->p.nz;
   const size_t n = s->n;
   const double D = s->p.mobility, kappa = 4.0 * s->p.mobility / s->p.width;
@@ -325,19 +334,39 @@ static void pass_allen_cahn(oracle_state *s) {
       for (int x = 0; x < nx; ++x) {
         size_t k = at(s, x, y, z);
         double adv = 0.0;
-        adv += face_flux(s, 0, x, y, z) - face_flux(s, 0, x - 1, y, z);
-        adv += face_flux(s, 1, x, y, z) - face_flux(s, 1, x, y - 1, z);
-        adv += face_flux(s, 2, x, y, z) - face_flux(s, 2, x, y, z - 1);
-        double lap = lap_at(s, s->phi, x, y, z);
+        adv += face_flux(s, phi, 0, x, y, z) - face_flux(s, phi, 0, x - 1, y, z);
+        adv += face_flux(s, phi, 1, x, y, z) - face_flux(s, phi, 1, x, y - 1, z);
+        adv += face_flux(s, phi, 2, x, y, z) - face_flux(s, phi, 2, x, y, z - 1);
+        double lap = lap_at(s, phi, x, y, z);
         double divq = 0.0;
         for (int i = 0; i < Q; ++i) {
           size_t kk = at(s, x + C[i][0], y + C[i][1], z + C[i][2]);
-          double ph = s->phi[kk];
-          for (int al = 0; al < 3; ++al) divq += W[i] * C[i][al] * (ph * (1.0 - ph) * s->nrm[al * n + kk]);
+          double ph = phi[kk];
+          for (int al = 0; al < 3; ++al) divq += W[i] * C[i][al] * (ph * (1.0 - ph) * nrm[al * n + kk]);
         }
         divq /= CS2;
-        s->phi2[k] = s->phi[k] + (-adv + D * lap - kappa * divq);
+        double euler = phi[k] + (-adv + D * lap - kappa * divq);
+        out[k] = base ? a * base[k] + b * euler : euler;
       }
+}
+
+/* Forward Euler (R13), or the three-stage SSP Runge-Kutta scheme of Shu and Osher (R32; PAPER.md:L110 names "time
+ * integrators" without choosing one) with the velocity frozen at u(t):
+ *   phi1 = phi + L(phi);  phi2 = 3/4 phi + 1/4 (phi1 + L(phi1));  phi(t+1) = 1/3 phi + 2/3 (phi2 + L(phi2)),
+ * the normal recomputed from every stage field. */
+static void pass_allen_cahn(oracle_state *s) {
+  if (!s->p.phi_rk3) {
+    allen_cahn_stage(s, s->phi, s->nrm, NULL, 0.0, 1.0, s->phi2);
+  } else {
+    allen_cahn_stage(s, s->phi, s->nrm, NULL, 0.0, 1.0, s->phi_s);               /* phi1 */
+    geometry_of(s, s->phi_s, NULL, s->nrm_s);
+    allen_cahn_stage(s, s->phi_s, s->nrm_s, s->phi, 0.75, 0.25, s->phi2);        /* phi2 */
+    geometry_of(s, s->phi2, NULL, s->nrm_s);
+    allen_cahn_stage(s, s->phi2, s->nrm_s, s->phi, 1.0 / 3.0, 2.0 / 3.0, s->phi_s); /* phi(t+1) */
+    double *t = s->phi_s;
+    s->phi_s = s->phi2;
+    s->phi2 = t;
+  }
   double *t = s->phi;
   s->phi = s->phi2;
   s->phi2 = t;
@@ -366,10 +395,15 @@ oracle_state *oracle_create(const oracle_params *p) {
     s->g = (double *)calloc(3 * n, sizeof(double));
     s->nrm = (double *)calloc(3 * n, sizeof(double));
     ok = ok && s->phi && s->phi2 && s->g && s->nrm;
+    if (p->phi_rk3) {
+      s->phi_s = (double *)calloc(n, sizeof(double));
+      s->nrm_s = (double *)calloc(3 * n, sizeof(double));
+      ok = ok && s->phi_s && s->nrm_s;
+    }
   }
   if (!ok) {
     free(s->f); free(s->pstar); free(s->u); free(s->a); free(s->A); free(s->m);
-    free(s->phi); free(s->phi2); free(s->g); free(s->nrm); free(s);
+    free(s->phi); free(s->phi2); free(s->g); free(s->nrm); free(s->phi_s); free(s->nrm_s); free(s);
     return NULL;
   }
   return s;
@@ -378,7 +412,7 @@ oracle_state *oracle_create(const oracle_params *p) {
 void oracle_destroy(oracle_state *s) {
   if (!s) return;
   free(s->f); free(s->pstar); free(s->u); free(s->a); free(s->A); free(s->m);
-  free(s->phi); free(s->phi2); free(s->g); free(s->nrm);
+  free(s->phi); free(s->phi2); free(s->g); free(s->nrm); free(s->phi_s); free(s->nrm_s);
   free(s);
 }
 
