@@ -342,6 +342,8 @@ def run_cuda(args):
     if barrier:
         barrier()
     cfg = make_workload(args.workload, args.n)
+    if args.rk3:
+        cfg["params"]["phi_rk3"] = 1
     meas = measure_cuda(cfg, args.steps, args.warmup, local_rank=local_rank, world=world, fp32=bool(args.fp32),
                         e2e=not args.no_e2e, variant=args.variant, barrier=barrier)
     # replicas only: every rank ran the same-sized independent problem; time = max over ranks
@@ -361,6 +363,7 @@ def run_cuda(args):
                                f"{'fp32' if args.fp32 else 'fp64'} population storage, fp64 arithmetic; "
                                + WORKLOADS[args.workload][1],
                    "n": args.n, "two_phase": two_phase, "population_storage": "fp32" if args.fp32 else "fp64",
+                   "phi_integrator": "ssp-rk3" if args.rk3 else "forward euler",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"state of {meas['workspace_bytes'] / 1e9:.1f} GB streams through a 126 MB L2 every step; no flush needed",
                    "lups_per_step": world * n3},
@@ -435,6 +438,7 @@ def main():
     ap.add_argument("--n", "--grid", dest="n", type=int, default=512, help="grid edge (default: the 512^3 the metric is quoted on)")
     ap.add_argument("--fp32", type=int, default=0, help="1: fp32 population storage (arithmetic stays fp64)")
     ap.add_argument("--variant", type=int, default=None, help="kernel variant (accLB_set_variant), default = best")
+    ap.add_argument("--rk3", type=int, default=0, help="1: SSP-RK3 integrator for phi (SURVEY 8(f) #1) instead of forward Euler")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-single", action="store_true", help="skip the single_phase leg of a two-phase run")

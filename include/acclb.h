@@ -60,6 +60,12 @@ typedef struct {
   int host_staging; /* 1: workspace also holds 5 n doubles of staging so accLB_run_host can be used        */
   int device;       /* CUDA device ordinal                                                                 */
   void* stream;     /* cudaStream_t of the caller (NULL = legacy default stream)                           */
+  /* the paper's two-component regime (density contrast 100, buoyant phase, time integrators) */
+  double gravity[3]; /* buoyancy F^g = (rho(phi) - rho_ref) g, a force density like the others (R3, R31)
+                        PAPER.md:L193, L203 ("buoyant gas phase"); single component: the uniform (1 - rho_ref) g   */
+  double rho_ref;    /* reference density of F^g; the mean density gives no net force on the periodic box (R31)   */
+  int phi_integrator; /* 0: forward Euler, once per LB step (R13) | 1: three-stage SSP Runge-Kutta with u frozen at
+                         time t, the normal recomputed from every stage field (R32)      */
 } accLB_params;
 
 /* Bytes of device workspace accLB_create needs for this grid and these parameters; 0 on invalid arguments
@@ -106,9 +112,9 @@ long long accLB_launch_count(const accLB_ctx* ctx);
  * record.  Kinds (the names are the kernels' own, as an ncu launch list shows them): 0 k_normal, 1 k_lb (the
  * one-node-per-thread fused LB step: single-phase default), 2 k_allen_cahn, 3 k_init, 4 k_moments, 5 k_diagnostics,
  * 6 k_lb_tp (the tiled two-phase step: LB + geometry + advection), 7 k_seam (advective fluxes through the seam faces
- * of its tile columns), 8 k_advect (variant 2 only).  This is how bench.py measures kernel durations inside the
- * timed region. */
-#define ACCLB_NKERNELS 9
+ * of its tile columns), 8 k_advect (variant 2 and the Runge-Kutta stages), 9 k_geom_r (D lap phi - kappa div q of a
+ * Runge-Kutta stage field).  This is how bench.py measures kernel durations inside the timed region. */
+#define ACCLB_NKERNELS 10
 int accLB_profile(accLB_ctx* ctx, int enable);
 int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
 

@@ -14,9 +14,9 @@ LIB_PATH = _PKG / "libacclb.so"
 HEADER = _PKG.parent / "include" / "acclb.h"
 
 NDIAG = 9
-NKERNELS = 9
+NKERNELS = 10
 KERNEL_NAMES = ("k_normal", "k_lb", "k_allen_cahn", "k_init", "k_moments", "k_diagnostics", "k_lb_tp", "k_seam",
-                "k_advect")
+                "k_advect", "k_geom_r")
 DIAG_NAMES = ("ke", "dissipation", "sum_phi", "sum_pstar", "sum_mx", "sum_my", "sum_mz", "umax", "step")
 ERRORS = {0: "ACCLB_OK", -1: "ACCLB_EINVAL", -2: "ACCLB_EWORKSPACE", -3: "ACCLB_ECUDA", -4: "ACCLB_ENUMERIC"}
 
@@ -36,6 +36,7 @@ class Params(C.Structure):
         ("force_type", C.c_int), ("force_amp", C.c_double), ("force_k", C.c_int),
         ("store_fp32", C.c_int), ("host_staging", C.c_int),
         ("device", C.c_int), ("stream", C.c_void_p),
+        ("gravity", C.c_double * 3), ("rho_ref", C.c_double), ("phi_integrator", C.c_int),
     ]
 
 
@@ -83,9 +84,11 @@ def _check(code):
 
 
 def make_params(*, tau, two_phase=0, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0, width=4.0, force_type=0,
-                force_amp=0.0, force_k=1, store_fp32=0, host_staging=0, device=0, stream=None):
+                force_amp=0.0, force_k=1, store_fp32=0, host_staging=0, device=0, stream=None,
+                gravity=(0.0, 0.0, 0.0), rho_ref=0.0, phi_rk3=0):
     return Params(tau, int(two_phase), rho_l, rho_g, sigma, mobility, width, int(force_type), force_amp, int(force_k),
-                  int(store_fp32), int(host_staging), int(device), stream)
+                  int(store_fp32), int(host_staging), int(device), stream, (C.c_double * 3)(*gravity), rho_ref,
+                  int(phi_rk3))
 
 
 def workspace_bytes(nx, ny, nz, params):

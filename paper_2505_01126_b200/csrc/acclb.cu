@@ -42,6 +42,8 @@ struct KP {
   int force_type;
   double force_amp;
   double nu, eps_pref;        // nu, nu / (2 cs4 tau^2) (R21)
+  double grav[3], rho_ref;    // buoyancy F^g = (rho - rho_ref) g       PAPER.md:L193, L203 (R31)
+  int buoyant;                // g != 0
 };
 
 // population storage: fp64, or fp32 deviation from the lattice weight (R22)
@@ -120,6 +122,10 @@ __device__ __forceinline__ void accel_from_gc(const KP& P, const Moments& M, con
   double F[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) F[a] = fs * g[a] + fp * g[a] + Fb[a];
+  if (P.buoyant) {  // F^g = (rho - rho_ref) g (R31)
+    const double dr = rho - P.rho_ref;
+    F[0] += dr * P.grav[0]; F[1] += dr * P.grav[1]; F[2] += dr * P.grav[2];
+  }
   if (with_visc && P.ratio_ne) {
     const double h = 0.5 / rho;
     const double ut[3] = {M.m[0] + F[0] * h, M.m[1] + F[1] * h, M.m[2] + F[2] * h};
@@ -152,6 +158,10 @@ __device__ __forceinline__ void node_accel(const KP& P, const double* __restrict
   if (!TWO_PHASE) {
     rho = 1.0;
     A[0] = Fb[0]; A[1] = Fb[1]; A[2] = Fb[2];
+    if (P.buoyant) {  // single component: the uniform acceleration (1 - rho_ref) g (R31)
+      const double dr = 1.0 - P.rho_ref;
+      A[0] += dr * P.grav[0]; A[1] += dr * P.grav[1]; A[2] += dr * P.grav[2];
+    }
     return;
   }
   const unsigned n = P.G.n;
@@ -442,6 +452,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
 }  // namespace acclb
 
 #include "twophase.cuh"
+#include "phase_rk.cuh"
 
 // ================================================================================================== host / ABI
 using namespace acclb;
@@ -457,6 +468,7 @@ struct accLB_ctx {
   double* phi[2];
   double* u;
   double* r;    // D lap phi - kappa div q of the current step (k_lb_tp -> k_advect)
+  double* phis; // RK3 only: the second stage field
   double* nrm;
   double* tabs;
   double* acc;
@@ -535,7 +547,7 @@ struct LaunchScope {
   }
 };
 enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_LB_TP = 6,
-       KIND_SEAM = 7, KIND_ADVECT = 8 };
+       KIND_SEAM = 7, KIND_ADVECT = 8, KIND_GEOM = 9 };
 
 static thread_local char g_err[512] = "";
 
@@ -556,6 +568,8 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
   if (27.0 * (double)nx * (double)ny >= 4294967296.0) return false;  // 32-bit offsets inside a [27][ny][nx] slab
   if (!(p->tau > 0.5) || !std::isfinite(p->tau)) return false;
   if (p->force_type < 0 || p->force_type > 2) return false;
+  if (!std::isfinite(p->gravity[0]) || !std::isfinite(p->gravity[1]) || !std::isfinite(p->gravity[2]) || !std::isfinite(p->rho_ref)) return false;
+  if (p->phi_integrator < 0 || p->phi_integrator > 1) return false;
   if (p->two_phase) {
     if (!(p->rho_l > 0.0) || !(p->rho_g > 0.0) || !(p->width > 0.0) || !(p->mobility >= 0.0)) return false;
   }
@@ -582,7 +596,7 @@ static int planes_per_block(int nx, int ny, int nz, int tx, int ty) {
 }
 
 struct Carve {
-  size_t f, phi, u, r, nrm, tabs, acc, sx, sy, sz, stage, total;
+  size_t f, phi, u, r, nrm, tabs, acc, sx, sy, sz, phis, stage, total;
 };
 static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   const size_t n = (size_t)nx * ny * nz;
@@ -600,8 +614,9 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   c.sx = p->two_phase ? align256((size_t)nz * ny * 2 * ntx * 8) : 0;
   c.sy = p->two_phase ? align256((size_t)nz * 2 * nty * nx * 8) : 0;
   c.sz = p->two_phase ? align256(2 * nchunk * (size_t)ny * nx * 8) : 0;
+  c.phis = p->two_phase && p->phi_integrator == 1 ? align256(n * 8) : 0;
   c.stage = p->host_staging ? align256(5 * n * 8) : 0;
-  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.sx + c.sy + c.sz + c.stage;
+  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.sx + c.sy + c.sz + c.phis + c.stage;
   return c;
 }
 
@@ -659,7 +674,8 @@ static int launch_seam(accLB_ctx* s, int c, int d) {
   return ACCLB_OK;
 }
 
-static int launch_advect(accLB_ctx* s, int c, int d) {
+static int launch_advect(accLB_ctx* s, const double* phi_in, double* phi_out, const double* base = nullptr, double ca = 0.0,
+                         double cb = 1.0) {
   using T = AdvTile<ADV_TX, ADV_TY>;
   auto kern = k_advect<ADV_TX, ADV_TY>;
   static thread_local int configured_device = -1;
@@ -670,7 +686,23 @@ static int launch_advect(accLB_ctx* s, int c, int d) {
   const int lz = planes_per_block(s->nx, s->ny, s->nz, ADV_TX, ADV_TY);
   const dim3 grid((s->nx + ADV_TX - 1) / ADV_TX, (s->ny + ADV_TY - 1) / ADV_TY, (s->nz + lz - 1) / lz);
   LaunchScope ls(s, KIND_ADVECT);
-  kern<<<grid, ADV_TX * ADV_TY, sizeof(T), s->stream>>>(s->kp, s->phi[c], s->u, s->r, s->phi[d], lz);
+  kern<<<grid, ADV_TX * ADV_TY, sizeof(T), s->stream>>>(s->kp, phi_in, s->u, s->r, phi_out, lz, base, ca, cb);
+  return ACCLB_OK;
+}
+
+// r = D lap phi - kappa div q of a Runge-Kutta stage field (k_geom_r, phase_rk.cuh).
+static int launch_geom_r(accLB_ctx* s, const double* phi_in) {
+  using T = GeomTile<LBT_TX, LBT_TY>;
+  auto kern = k_geom_r<LBT_TX, LBT_TY>;
+  static thread_local int configured_device = -1;
+  if (configured_device != s->prm.device) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
+    configured_device = s->prm.device;
+  }
+  const int lz = s->lz;
+  const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
+  LaunchScope ls(s, KIND_GEOM);
+  kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, phi_in, s->r, lz);
   return ACCLB_OK;
 }
 
@@ -753,6 +785,7 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   s->seams.ntx = (nx + LBT_TX - 1) / LBT_TX;
   s->seams.nty = (ny + LBT_TY - 1) / LBT_TY;
   s->lz = planes_per_block(nx, ny, nz, LBT_TX, LBT_TY);
+  s->phis = c.phis ? (double*)w : nullptr; w += c.phis;
   s->stage = p->host_staging ? (double*)w : nullptr; w += c.stage;
   s->cur = 0; s->step = 0; s->launches = 0; s->variant = 0; s->profiling = 0;
   for (int k = 0; k < ACCLB_NKERNELS; ++k) { s->folded_ms[k] = 0.0; s->folded_count[k] = 0; }
@@ -770,6 +803,9 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   k.kappa = p->two_phase ? 4.0 * p->mobility / p->width : 0.0;
   k.force_type = p->force_type;
   k.force_amp = p->force_amp;
+  for (int a = 0; a < 3; ++a) k.grav[a] = p->gravity[a];
+  k.rho_ref = p->rho_ref;
+  k.buoyant = p->gravity[0] != 0.0 || p->gravity[1] != 0.0 || p->gravity[2] != 0.0;
   k.nu = (p->tau - 0.5) / 3.0;
   k.eps_pref = k.nu / (2.0 * (1.0 / 9.0) * p->tau * p->tau);
 
@@ -838,7 +874,16 @@ int accLB_step(accLB_ctx* s, int nsteps) {
   const unsigned nb = blocks_for(s->n, 128);
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
-    if (s->prm.two_phase && s->variant == 0) {
+    if (s->prm.two_phase && s->prm.phi_integrator == 1) {
+      // SSP-RK3 for phi (R32): LB with u(t), r(phi) through HBM, then three Allen-Cahn stages with u frozen
+      int r = launch_lb_tp_any<false>(s, c, d);
+      if (r) return r;
+      if ((r = launch_advect(s, s->phi[c], s->phi[d]))) return r;                                  // phi1 -> phi[d]
+      if ((r = launch_geom_r(s, s->phi[d]))) return r;
+      if ((r = launch_advect(s, s->phi[d], s->phis, s->phi[c], 0.75, 0.25))) return r;             // phi2 -> phis
+      if ((r = launch_geom_r(s, s->phis))) return r;
+      if ((r = launch_advect(s, s->phis, s->phi[d], s->phi[c], 1.0 / 3.0, 2.0 / 3.0))) return r;   // phi(t+1) -> phi[d]
+    } else if (s->prm.two_phase && s->variant == 0) {
       // default: LB + geometry + advection fused on z-marching tiles (k_lb_tp), then the seam faces (k_seam)
       int r = launch_lb_tp_any<true>(s, c, d);
       if (r) return r;
@@ -848,7 +893,7 @@ int accLB_step(accLB_ctx* s, int nsteps) {
       // variant 2: round 1's two-kernel form, u and r through HBM (k_lb_tp<unfused>, k_advect)
       int r = launch_lb_tp_any<false>(s, c, d);
       if (r) return r;
-      r = launch_advect(s, c, d);
+      r = launch_advect(s, s->phi[c], s->phi[d]);
       if (r) return r;
     } else if (s->prm.two_phase) {
       // variant 1: one node per thread, stencils straight from global memory (k_normal, k_lb, k_allen_cahn)

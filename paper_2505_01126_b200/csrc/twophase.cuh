@@ -119,7 +119,8 @@ struct GeoTile {
   unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
-  static constexpr int NR = FUSED ? 5 : 4;
+  static constexpr int NR = 5;  // (five also without the fused advection: phi(z) is read after the last barrier of an iteration,
+                                // so the slot of plane zc-2 must not be the landing slot of the next iteration's fetch)
   alignas(16) double raw[NR][PY][PX];  // ring of raw phi planes (zc-2,) zc-1, zc, zc+1 and zc+2 (landing, cp.async)
   alignas(16) double2 nq[3][NY][NX];  // (n_c, q_c), c = x, y, z, of plane zc, q = phi (1 - phi) n: one 16-byte access serves both
   double ftab[2][LZ_MAX]; // sin / cos force table entries of this block's planes (lz <= LZ_MAX): the streaming pulls evict
@@ -655,7 +656,7 @@ struct AdvTile {
 template <int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 4)
 k_advect(KP P, const double* __restrict__ phi, const double* __restrict__ u, const double* __restrict__ r,
-         double* __restrict__ phi_new, int lz) {
+         double* __restrict__ phi_new, int lz, const double* __restrict__ base, double ca, double cb) {
   using T = AdvTile<TX, TY>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
@@ -765,7 +766,9 @@ k_advect(KP P, const double* __restrict__ phi, const double* __restrict__ u, con
       adv += S.fx[ty][tx + 1] - S.fx[ty][tx];
       adv += S.fy[ty + 1][tx] - S.fy[ty][tx];
       adv += fz - fz_prev;
-      __stcs(phi_new + (size_t)z * plane + own, w2 + (-adv + rr));
+      const double euler = w2 + (-adv + rr);
+      // a Runge-Kutta stage (phase_rk.cuh) combines the Euler update of the stage field with the base field phi(t)
+      __stcs(phi_new + (size_t)z * plane + own, base ? ca * __ldg(base + (size_t)z * plane + own) + cb * euler : euler);
     }
     fz_prev = fz;
   }

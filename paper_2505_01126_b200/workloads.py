@@ -40,13 +40,12 @@ _VELOCITY_CACHE = {}
 
 def hit_velocity(n, urms=0.03, seed=SEED_VELOCITY, k_peak=4.0):
     """Configs 2/4/5: seeded random solenoidal field with shell spectrum E(k) ~ k^4 exp(-2 (k/k_peak)^2),
-    normalised to sqrt(<u.u>/3) = urms (R28).  The last field is kept (read-only): configs 2 and 4 of one size share it."""
+    normalised to sqrt(<u.u>/3) = urms (R28).  The last field is kept (callers must not modify it): configs 2 and 4 of one size share it."""
     key = (n, urms, seed, k_peak)
     if key in _VELOCITY_CACHE:
         return _VELOCITY_CACHE[key]
     _VELOCITY_CACHE.clear()
     u = _hit_velocity(n, urms, seed, k_peak)
-    u.setflags(write=False)
     _VELOCITY_CACHE[key] = u
     return u
 

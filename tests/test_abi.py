@@ -32,7 +32,7 @@ def test_params_struct_matches_header():
     text = binding.HEADER.read_text()
     body = re.search(r"typedef struct \{(.*?)\} accLB_params;", text, flags=re.S).group(1)
     body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
-    fields = re.findall(r"\b(?:double|int|void\*)\s+(\w+);", body)
+    fields = re.findall(r"\b(?:double|int|void\*)\s+(\w+)(?:\[\d+\])?;", body)
     assert fields == [f[0] for f in binding.Params._fields_]
 
 
