@@ -653,24 +653,20 @@ static int launch_lb_tp_any(accLB_ctx* s, int c, int d) {
   return launch_lb_tp<double, FUSED, false>(s, c, d);
 }
 
-// The fluxes through the seam faces of the tile columns (k_seam: one launch per direction), after k_lb_tp<FUSED> of the
-// same step.
+// The fluxes through the seam faces of the tile columns (k_seam: one launch for the three directions), after
+// k_lb_tp<FUSED> of the same step.
 static int launch_seam(accLB_ctx* s, int c, int d) {
-  const int nchunk = (s->nz + s->lz - 1) / s->lz;
-  const size_t nfx = (size_t)s->seams.ntx * s->ny * s->nz, nfy = (size_t)s->nx * s->seams.nty * s->nz,
-               nfz = (size_t)s->nx * s->ny * nchunk;
-  {
-    LaunchScope ls(s, KIND_SEAM);
-    k_seam<1><<<blocks_for(nfy, 128), 128, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, LBT_TY, s->seams.nty, (unsigned)nfy);
-  }
-  {
-    LaunchScope ls(s, KIND_SEAM);
-    k_seam<0><<<blocks_for(nfx, 128), 128, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, LBT_TX, s->seams.ntx, (unsigned)nfx);
-  }
-  {
-    LaunchScope ls(s, KIND_SEAM);
-    k_seam<2><<<blocks_for(nfz, 128), 128, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, s->lz, nchunk, (unsigned)nfz);
-  }
+  SeamGrid g;
+  g.lz = s->lz;
+  g.nchunk = (s->nz + s->lz - 1) / s->lz;
+  g.nfx = (unsigned)((size_t)s->seams.ntx * s->ny * s->nz);
+  g.nfy = (unsigned)((size_t)s->nx * s->seams.nty * s->nz);
+  g.nfz = (unsigned)((size_t)s->nx * s->ny * g.nchunk);
+  g.bx = blocks_for(g.nfx, SEAM_THREADS);
+  g.by = blocks_for(g.nfy, SEAM_THREADS);
+  g.bz = blocks_for(g.nfz, SEAM_THREADS);
+  LaunchScope ls(s, KIND_SEAM);
+  k_seam<LBT_TX, LBT_TY><<<g.bx + g.by + g.bz, SEAM_THREADS, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, g);
   return ACCLB_OK;
 }
 

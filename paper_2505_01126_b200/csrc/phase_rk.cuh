@@ -81,7 +81,7 @@ k_geom_r(KP P, const double* __restrict__ phi, double* __restrict__ rout, int lz
       const double gx = (1.0 / 72.0) * fma(4.0, t[5] - t[3], (t[2] - t[0]) + (t[8] - t[6]));
       const double gy = (1.0 / 72.0) * fma(4.0, t[7] - t[1], (t[6] - t[0]) + (t[8] - t[2]));
       const double gz = (1.0 / 72.0) * fma(4.0, fma(4.0, d[4], d[3] + d[5]), fma(4.0, d[1], d[0] + d[2]) + fma(4.0, d[7], d[6] + d[8]));
-      const double gn = sqrt(fma(gx, gx, fma(gy, gy, gz * gz)));
+      const double gn = sqrt_pos(fma(gx, gx, fma(gy, gy, gz * gz)));
       const double pq = ph * (1.0 - ph) * div_pos(1.0, gn + 1e-12);
       S.q[0][j][i] = pq * gx;
       S.q[1][j][i] = pq * gy;

@@ -99,6 +99,20 @@ __device__ __forceinline__ double laplacian27(const double (&v)[3][3][3]) {
   return 6.0 * (acc * (1.0 / 216.0) - v[1][1][1]);
 }
 
+// sqrt(s) for s >= 0: hardware reciprocal-square-root seed, two Newton steps on y ~ 1/sqrt(s), then s y with one residual
+// correction; relative error ~1e-16, a fixed instruction sequence without the library routine's special-case call.
+// s = 0 gives 0 (the seed is taken of max(s, 1e-300); below that the result is only needed to be << 1e-12, R17).
+__device__ __forceinline__ double sqrt_pos(double s) {
+  double y;
+  const double sc = fmax(s, 1e-300);
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(sc));
+  const double h = 0.5 * sc;
+  y = __fma_rn(__fma_rn(-h * y, y, 0.5), y, y);
+  y = __fma_rn(__fma_rn(-h * y, y, 0.5), y, y);
+  const double r = s * y;
+  return __fma_rn(__fma_rn(-r, r, s), 0.5 * y, r);
+}
+
 // a / b for b > 0 in the normal range: hardware reciprocal seed (relative error 2^-23), two Newton steps and one
 // residual correction of the quotient; within an ulp of the correctly rounded quotient, a fixed instruction sequence
 // (so both cells of a face get the same bits), about half the instructions of the IEEE division with its slow path.
@@ -131,14 +145,12 @@ __device__ __forceinline__ double weno5_minus_c(double d1, double d2, double d3,
   const double r1 = __fma_rn(13.0, __dmul_rn(s1, s1), __fma_rn(3.0, __dmul_rn(t1, t1), eps12));
   const double r2 = __fma_rn(13.0, __dmul_rn(s2, s2), __fma_rn(3.0, __dmul_rn(t2, t2), eps12));
   const double e0 = __dmul_rn(r0, r0), e1 = __dmul_rn(r1, r1), e2 = __dmul_rn(r2, r2);
-  const double n0 = __dmul_rn(0.1, __dmul_rn(e1, e2));
-  const double n1 = __dmul_rn(0.6, __dmul_rn(e0, e2));
-  const double n2 = __dmul_rn(0.3, __dmul_rn(e0, e1));
-  const double x0 = __fma_rn(5.0, d2, __dmul_rn(-2.0, d1));  // 6 (q0 - c)
-  const double x1 = __fma_rn(2.0, d3, d2);                   // 6 (q1 - c)
-  const double x2 = __fma_rn(4.0, d3, -d4);                  // 6 (q2 - c)
-  const double num = __fma_rn(n2, x2, __fma_rn(n1, x1, __dmul_rn(n0, x0)));
-  const double den = __dmul_rn(6.0, __dadd_rn(__dadd_rn(n0, n1), n2));
+  const double m0 = __dmul_rn(e1, e2), m1 = __dmul_rn(e0, e2), m2 = __dmul_rn(e0, e1);  // weights d_k m_k, d = (.1,.6,.3)
+  const double x0 = __fma_rn(0.5, d2, __dmul_rn(-0.2, d1));  // 0.1 * 6 (q0 - c)
+  const double x1 = __fma_rn(1.2, d3, __dmul_rn(0.6, d2));   // 0.6 * 6 (q1 - c)
+  const double x2 = __fma_rn(1.2, d3, __dmul_rn(-0.3, d4));  // 0.3 * 6 (q2 - c)
+  const double num = __fma_rn(m2, x2, __fma_rn(m1, x1, __dmul_rn(m0, x0)));
+  const double den = __fma_rn(1.8, m2, __fma_rn(3.6, m1, __dmul_rn(0.6, m0)));  // 6 (0.1 m0 + 0.6 m1 + 0.3 m2)
   return div_pos(num, den);
 }
 

@@ -13,9 +13,9 @@
 //               phi(t+1) = phi + r - sum_e (Phi_e(x) - Phi_e(x - e)) without the faces on the tile's seams, whose second
 //               velocity belongs to another block; the velocities on the seams go to three thin strips (2.6 B per node).
 //   k_seam      adds the fluxes through the seam faces (x = multiples of TX, y = multiples of TY, z = multiples of lz:
-//               5 % of all faces) to the cells on either side, from the strips and phi(t).  Every cell gathers its own
-//               seam faces with the same explicitly rounded instruction sequence, so a face's flux has identical bits
-//               on both sides and sum phi is conserved to rounding (R12) without atomics.
+//               5 % of all faces) to the cells on either side, from the strips and phi(t): one thread per face, one
+//               flux per face, added to one cell and subtracted from the other (atomics): sum phi is conserved to
+//               rounding (R12).
 //   FUSED = false + k_advect is the round-1 two-kernel form (u, r through HBM), kept as variant 2 for comparison:
 //   k_advect    the advective part of a8: phi+ = phi + (-sum_e (Phi_e(x) - Phi_e(x - e)) + r); every face flux is
 //               computed once per face (shared memory for x / y faces, a register carried along z for z faces).
@@ -404,7 +404,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const double r1 = fma(4.0, d[4], d[3] + d[5]);
         const double r2_ = fma(4.0, d[7], d[6] + d[8]);
         const double gz = (1.0 / 72.0) * fma(4.0, r1, r0 + r2_);
-        const double gn = sqrt(fma(gx, gx, fma(gy, gy, gz * gz)));
+        const double gn = sqrt_pos(fma(gx, gx, fma(gy, gy, gz * gz)));
         const double inv = div_pos(1.0, gn + 1e-12);
         const double pq = ph * (1.0 - ph);
         const double nx_ = gx * inv, ny_ = gy * inv, nz_ = gz * inv;
@@ -592,49 +592,67 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
 
 // a8 on the seams of the tile columns of k_lb_tp<FUSED> (R12).  A face is a seam when its two cells
 // belong to different tile columns / z chunks: x faces in front of x = TX b, y faces in front of y = TY b, z faces in
-// front of z = lz b (b = 0 is the periodic wrap).  One launch per direction DIR (0: x, 1: y, 2: z), one thread per seam
-// face: it evaluates the flux once from the two strip velocities and phi(t) and adds it to phi(t+1) of the cell behind
-// the face (+) and of the cell in front (-), so sum phi is conserved to rounding.  All updates of one cell within a launch
-// come from one thread (a tile only one cell thick gets both of its faces from the thread of its lower face), and the
-// three launches are ordered on the stream: no atomics, bitwise reproducible.
-template <int DIR>
-__global__ void __launch_bounds__(128) k_seam(KP P, const double* __restrict__ phi, double* __restrict__ phi_new, Seams SM,
-                                              int tile, int ntile, unsigned nfaces) {
+// front of z = lz b (b = 0 is the periodic wrap).  ONE launch for the three directions, one thread per seam face: it
+// evaluates the flux once from the two strip velocities and phi(t) and adds it to phi(t+1) of the cell in front of the
+// face (+) and subtracts it from the cell behind (-), so sum phi is conserved to rounding.  The additions are atomic: a
+// cell on a tile edge receives fluxes from two or three seams, in an order that is not fixed (last-bit differences from
+// run to run in those cells; every other cell is bitwise reproducible).  The blocks of the x faces (latency-bound: their
+// cells are a tile width apart) are interleaved with those of the y faces (bandwidth-bound: whole rows) so that the two
+// kinds overlap on every SM; lanes run along y for the x faces (the strips u_x[z][bx][y][s] are then contiguous) and
+// along x for the y and z faces.
+constexpr int SEAM_THREADS = 128;
+struct SeamGrid {
+  unsigned nfx, nfy, nfz;  // seam faces per direction
+  unsigned bx, by, bz;     // blocks per direction
+  int lz, nchunk;
+};
+template <int TX, int TY>
+__global__ void __launch_bounds__(SEAM_THREADS) k_seam(KP P, const double* __restrict__ phi, double* __restrict__ phi_new,
+                                                       Seams SM, SeamGrid SG) {
   const Grid& G = P.G;
-  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nfaces) return;
   const size_t plane = (size_t)G.nx * (size_t)G.ny;
-  const int n = DIR == 0 ? G.nx : DIR == 1 ? G.ny : G.nz;  // extent along DIR
-  int x, y, z, b;                                           // b: tile whose first cell lies behind the face
-  if (DIR == 0) {
-    b = (int)(t % (unsigned)ntile);
-    const unsigned r = t / (unsigned)ntile;
-    y = (int)(r % (unsigned)G.ny); z = (int)(r / (unsigned)G.ny); x = b * tile;
-  } else if (DIR == 1) {
-    x = (int)(t % (unsigned)G.nx);
-    const unsigned r = t / (unsigned)G.nx;
-    b = (int)(r % (unsigned)ntile); z = (int)(r / (unsigned)ntile); y = b * tile;
+  // which direction this block serves: x and y blocks interleaved in proportion, z blocks last
+  const unsigned i = blockIdx.x, T = SG.bx + SG.by;
+  int dir;
+  unsigned blk;
+  if (i < T) {
+    const unsigned y0 = (unsigned)(((unsigned long long)i * SG.by) / T), y1 = (unsigned)(((unsigned long long)(i + 1) * SG.by) / T);
+    if (y1 > y0) { dir = 1; blk = y0; }
+    else { dir = 0; blk = i - y1; }
   } else {
-    x = (int)(t % (unsigned)G.nx);
+    dir = 2; blk = i - T;
+  }
+  const unsigned t = blk * SEAM_THREADS + threadIdx.x;
+  if (dir == 0) {
+    if (t >= SG.nfx) return;
+    const int y = (int)(t % (unsigned)G.ny);
+    const unsigned r = t / (unsigned)G.ny;
+    const int b = (int)(r % (unsigned)SM.ntx), z = (int)(r / (unsigned)SM.ntx);
+    const int c0 = b * TX, bp = b == 0 ? SM.ntx - 1 : b - 1;
+    const double F = seam_face_flux<0>(G, phi, SM, 0, y, z, c0, b, bp);
+    double* row = phi_new + (size_t)z * plane + (size_t)y * G.nx;
+    atomicAdd(row + c0, F);
+    atomicAdd(row + (c0 == 0 ? G.nx - 1 : c0 - 1), -F);
+  } else if (dir == 1) {
+    if (t >= SG.nfy) return;
+    const int x = (int)(t % (unsigned)G.nx);
     const unsigned r = t / (unsigned)G.nx;
-    y = (int)(r % (unsigned)G.ny); b = (int)(r / (unsigned)G.ny); z = b * tile;
-  }
-  const int c0 = b * tile;  // coordinate along DIR of the first cell in front of the face
-  const int bp = b == 0 ? ntile - 1 : b - 1, bn = b == ntile - 1 ? 0 : b + 1;
-  const size_t stride = DIR == 0 ? 1 : DIR == 1 ? (size_t)G.nx : plane;
-  const size_t base = (size_t)z * plane + (size_t)y * G.nx + x - (size_t)c0 * stride;  // cell with coordinate 0 along DIR
-  const double F = seam_face_flux<DIR>(G, phi, SM, x, y, z, c0, b, bp);
-  double dR = F;
-  if (min(tile, n - c0) == 1) {  // one-cell tile: its upper face too
-    auto ph = [&](int k) { return __ldg(phi + base + (size_t)wrap_add(c0, k, n) * stride); };
-    dR -= face_flux(seam_vel<DIR>(SM, G, x, y, z, b, 1), seam_vel<DIR>(SM, G, x, y, z, bn, 0), ph(-2), ph(-1), ph(0), ph(1),
-                    ph(2), ph(3));
-  }
-  double* const cR = phi_new + base + (size_t)c0 * stride;
-  *cR = *cR + dR;
-  if (min(tile, n - bp * tile) > 1) {
-    double* const cL = phi_new + base + (size_t)wrap_add(c0, -1, n) * stride;
-    *cL = *cL - F;
+    const int b = (int)(r % (unsigned)SM.nty), z = (int)(r / (unsigned)SM.nty);
+    const int c0 = b * TY, bp = b == 0 ? SM.nty - 1 : b - 1;
+    const double F = seam_face_flux<1>(G, phi, SM, x, 0, z, c0, b, bp);
+    double* col = phi_new + (size_t)z * plane + x;
+    atomicAdd(col + (size_t)c0 * G.nx, F);
+    atomicAdd(col + (size_t)(c0 == 0 ? G.ny - 1 : c0 - 1) * G.nx, -F);
+  } else {
+    if (t >= SG.nfz) return;
+    const int x = (int)(t % (unsigned)G.nx);
+    const unsigned r = t / (unsigned)G.nx;
+    const int y = (int)(r % (unsigned)G.ny), b = (int)(r / (unsigned)G.ny);
+    const int c0 = b * SG.lz, bp = b == 0 ? SG.nchunk - 1 : b - 1;
+    const double F = seam_face_flux<2>(G, phi, SM, x, y, 0, c0, b, bp);
+    double* cell = phi_new + (size_t)y * G.nx + x;
+    atomicAdd(cell + (size_t)c0 * plane, F);
+    atomicAdd(cell + (size_t)(c0 == 0 ? G.nz - 1 : c0 - 1) * plane, -F);
   }
 }
 
