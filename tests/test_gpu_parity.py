@@ -264,17 +264,18 @@ def test_moments_leave_state_unchanged_and_step_counts(acclb):
     a.diagnostics()
     a.step(2)
     b.step(5)
+    same = lambda x, y: (x - y).abs().max().item() <= 1e-14   # bitwise but for the cells on tile edges (atomic adds in k_seam)
     for x, y in zip(a.moments(), b.moments()):
-        assert torch.equal(x, y)
+        assert same(x, y)
     assert a.diagnostics()["step"] == 5
-    # re-init restarts the clock and reproduces the run bit for bit
+    # re-init restarts the clock and reproduces the run
     first = [t.clone() for t in b.moments()]
     dev = b.device
     b.init(torch.from_numpy(cfg["rho"]).to(dev), torch.from_numpy(cfg["u"]).to(dev), torch.from_numpy(cfg["phi"]).to(dev))
     assert b.diagnostics()["step"] == 0
     b.step(5)
     for x, y in zip(first, b.moments()):
-        assert torch.equal(x, y)
+        assert same(x, y)
 
 
 def test_run_host_equals_device_path(acclb):
@@ -287,7 +288,10 @@ def test_run_host_equals_device_path(acclb):
     rho_o, u_o, phi_o = torch.empty(n, n, n, dtype=torch.float64), torch.empty(3, n, n, n, dtype=torch.float64), torch.empty(n, n, n, dtype=torch.float64)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     d = sim.run_host(pin(cfg["rho"]), pin(cfg["u"]), pin(cfg["phi"]), 7, rho_o, u_o, phi_o)
-    assert torch.equal(rho_o, ref[0]) and torch.equal(u_o, ref[1]) and torch.equal(phi_o, ref[2])
+    # the same path on the same inputs: identical up to the order of the atomic flux additions into the cells on tile edges
+    # (k_seam: last-bit differences in phi there, which the forces carry into p* and u)
+    for got, want in ((rho_o, ref[0]), (u_o, ref[1]), (phi_o, ref[2])):
+        assert (got - want).abs().max().item() <= 1e-14
     assert d["step"] == 7 and abs(d["sum_phi"] - dref["sum_phi"]) <= 1e-12 * dref["sum_phi"]
     plain = gpu_sim(acclb, cfg)
     with pytest.raises(acclb.AccLBError):
