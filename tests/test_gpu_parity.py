@@ -308,7 +308,7 @@ def test_launch_count_and_errors(acclb):
     sim2 = gpu_sim(acclb, cfg2)
     c0 = sim2.launch_count
     sim2.step(4)
-    assert sim2.launch_count - c0 == 16        # LB + geometry + advection fused on tiles, then the seam faces (x, y, z)
+    assert sim2.launch_count - c0 == 8         # LB + geometry + advection fused on tiles, then the seam faces (one launch)
     sim2.set_variant(2)
     c0 = sim2.launch_count
     sim2.step(4)
