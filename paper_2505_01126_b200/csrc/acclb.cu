@@ -628,10 +628,13 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
 
 static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
-template <typename ST, bool FUSED, bool FAST>
-static int launch_lb_tp(accLB_ctx* s, int c, int d) {
-  using T = GeoTile<ST, LBT_TX, LBT_TY, FUSED>;
-  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB, FUSED, FAST>;
+// One launch of the tiled two-phase kernel in the given MODE (twophase.cuh) on the state f[c], phi[c]; f[d], phi[d] are the
+// targets of a step.  out_u / out_r / in0 / in1: see the MODE list.
+template <typename ST, int MODE, bool FAST>
+static int launch_lb_tp(accLB_ctx* s, int c, int d, int kind, double* out_u, double* out_r, const double* in0,
+                        const double* in1) {
+  using T = GeoTile<ST, LBT_TX, LBT_TY, MODE == MODE_FUSED>;
+  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB, MODE, FAST>;
   static thread_local int configured_device = -1;
   if (configured_device != s->prm.device) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
@@ -639,18 +642,20 @@ static int launch_lb_tp(accLB_ctx* s, int c, int d) {
   }
   const int lz = s->lz;
   const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
-  LaunchScope ls(s, KIND_LB_TP);
-  kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], s->u, s->r,
-                                                        s->phi[d], s->seams, s->tabs, lz, s->tmap[c], s->tmap_row[c]);
+  LaunchScope ls(s, kind);
+  kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], out_u, out_r,
+                                                        s->phi[d], s->seams, s->tabs, lz, s->tmap[c], s->tmap_row[c], in0, in1);
   return ACCLB_OK;
 }
 
 // FAST (all tiles full, TMA pull) when the tensor maps exist and the tile shape divides the box; fp64 storage only.
-template <bool FUSED>
-static int launch_lb_tp_any(accLB_ctx* s, int c, int d) {
-  if (s->prm.store_fp32) return launch_lb_tp<float, FUSED, false>(s, c, d);
-  if (s->tmap_ok) return launch_lb_tp<double, FUSED, true>(s, c, d);
-  return launch_lb_tp<double, FUSED, false>(s, c, d);
+template <int MODE>
+static int launch_lb_tp_any(accLB_ctx* s, int c, int d, int kind = KIND_LB_TP, double* out_u = nullptr,
+                            double* out_r = nullptr, const double* in0 = nullptr, const double* in1 = nullptr) {
+  if (MODE == MODE_UNFUSED) { out_u = s->u; out_r = s->r; }
+  if (s->prm.store_fp32) return launch_lb_tp<float, MODE, false>(s, c, d, kind, out_u, out_r, in0, in1);
+  if (MODE != MODE_INIT && s->tmap_ok) return launch_lb_tp<double, MODE, MODE != MODE_INIT>(s, c, d, kind, out_u, out_r, in0, in1);
+  return launch_lb_tp<double, MODE, false>(s, c, d, kind, out_u, out_r, in0, in1);
 }
 
 // The fluxes through the seam faces of the tile columns (k_seam: one launch for the three directions), after
@@ -845,14 +850,10 @@ int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* p
   s->step = 0;
   const unsigned nb = blocks_for(s->n, 128);
   if (s->prm.two_phase) {
+    // the tiled kernel in MODE_INIT: geometry of phi on shared-memory tiles, f_i pushed to x - c_i
     CK(cudaMemcpyAsync(s->phi[0], phi, s->n * 8, cudaMemcpyDeviceToDevice, s->stream));
-    int r = launch_normal(s);
+    int r = launch_lb_tp_any<MODE_INIT>(s, 0, 0, KIND_INIT, nullptr, nullptr, rho, u);
     if (r) return r;
-    LaunchScope ls(s, KIND_INIT);
-    if (s->prm.store_fp32)
-      k_init<float, true><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, s->phi[0], s->nrm, s->tabs, (float*)s->f[0]);
-    else
-      k_init<double, true><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, s->phi[0], s->nrm, s->tabs, (double*)s->f[0]);
   } else {
     LaunchScope ls(s, KIND_INIT);
     if (s->prm.store_fp32)
@@ -872,7 +873,7 @@ int accLB_step(accLB_ctx* s, int nsteps) {
     const int c = s->cur, d = c ^ 1;
     if (s->prm.two_phase && s->prm.phi_integrator == 1) {
       // SSP-RK3 for phi (R32): LB with u(t), r(phi) through HBM, then three Allen-Cahn stages with u frozen
-      int r = launch_lb_tp_any<false>(s, c, d);
+      int r = launch_lb_tp_any<MODE_UNFUSED>(s, c, d);
       if (r) return r;
       if ((r = launch_advect(s, s->phi[c], s->phi[d]))) return r;                                  // phi1 -> phi[d]
       if ((r = launch_geom_r(s, s->phi[d]))) return r;
@@ -881,13 +882,13 @@ int accLB_step(accLB_ctx* s, int nsteps) {
       if ((r = launch_advect(s, s->phis, s->phi[d], s->phi[c], 1.0 / 3.0, 2.0 / 3.0))) return r;   // phi(t+1) -> phi[d]
     } else if (s->prm.two_phase && s->variant == 0) {
       // default: LB + geometry + advection fused on z-marching tiles (k_lb_tp), then the seam faces (k_seam)
-      int r = launch_lb_tp_any<true>(s, c, d);
+      int r = launch_lb_tp_any<MODE_FUSED>(s, c, d);
       if (r) return r;
       r = launch_seam(s, c, d);
       if (r) return r;
     } else if (s->prm.two_phase && s->variant == 2) {
       // variant 2: round 1's two-kernel form, u and r through HBM (k_lb_tp<unfused>, k_advect)
-      int r = launch_lb_tp_any<false>(s, c, d);
+      int r = launch_lb_tp_any<MODE_UNFUSED>(s, c, d);
       if (r) return r;
       r = launch_advect(s, s->phi[c], s->phi[d]);
       if (r) return r;
@@ -926,14 +927,9 @@ int accLB_moments(accLB_ctx* s, double* rho, double* u, double* phi) {
   const unsigned nb = blocks_for(s->n, 128);
   const int c = s->cur;
   if (s->prm.two_phase) {
-    int r = launch_normal(s);
-    if (r) return r;
-    {
-      LaunchScope ls(s, KIND_MOMENTS);
-      if (s->prm.store_fp32)
-        k_moments<float, true><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], s->phi[c], s->nrm, s->tabs, rho, u);
-      else
-        k_moments<double, true><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], s->phi[c], s->nrm, s->tabs, rho, u);
+    if (rho || u) {
+      int r = launch_lb_tp_any<MODE_MOMENTS>(s, c, c, KIND_MOMENTS, u, rho);
+      if (r) return r;
     }
     if (phi) CK(cudaMemcpyAsync(phi, s->phi[c], s->n * 8, cudaMemcpyDeviceToDevice, s->stream));
   } else {
@@ -956,13 +952,8 @@ int accLB_diagnostics(accLB_ctx* s, double* out, int n_out) {
   const unsigned cap = 148u * 16u;  // a multiple of the SM count; grid-stride beyond that
   if (nb > cap) nb = cap;
   if (s->prm.two_phase) {
-    int r = launch_normal(s);
+    int r = launch_lb_tp_any<MODE_DIAG>(s, c, c, KIND_DIAG, nullptr, s->acc);
     if (r) return r;
-    LaunchScope ls(s, KIND_DIAG);
-    if (s->prm.store_fp32)
-      k_diagnostics<float, true><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const float*)s->f[c], s->phi[c], s->nrm, s->tabs, s->acc);
-    else
-      k_diagnostics<double, true><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const double*)s->f[c], s->phi[c], s->nrm, s->tabs, s->acc);
   } else {
     LaunchScope ls(s, KIND_DIAG);
     if (s->prm.store_fp32)

@@ -181,13 +181,31 @@ __device__ __forceinline__ double seam_face_flux(const Grid& G, const double* __
 // fp64 work instead of stalling every warp at the top of the node update, and no register holds a load in flight.
 // FAST (fp64 storage, nx a multiple of TX, ny a multiple of TY, tensor maps available): every tile is full and pulls by
 // TMA; no thread is idle and no per-thread wrap tables are kept.  Otherwise every tile pulls with per-thread cp.async.
-template <typename ST, int TX, int TY, int MINB, bool FUSED, bool FAST>
+// MODE: what a node does with its moments and its force -- the march, the staging and the geometry are the same:
+//   MODE_FUSED    the time step (default): collide + store, advection fused, seam strips            rows a1-a8
+//   MODE_UNFUSED  the time step with u(t) -> uout and r -> rout for k_advect (variant 2, RK3 stages)  rows a1-a7
+//   MODE_MOMENTS  accLB_moments: p* -> rout, u -> uout (either may be NULL); the state is not touched   row a9
+//   MODE_DIAG     accLB_diagnostics: the sums of R21 -> rout[0..7] (warp shuffle + one atomic per block and quantity)
+//   MODE_INIT     accLB_init (R15): no pull; p* = in0, u0 = in1, A from F^s + F^p + F^b + F^g (F^nu := 0),
+//                 f_i = f_i^eq(p*, u0) - S_i(u0, A)/2 written "pushed" to x - c_i so that the first pull returns it at x
+enum { MODE_FUSED = 0, MODE_UNFUSED = 1, MODE_MOMENTS = 2, MODE_DIAG = 3, MODE_INIT = 4 };
+
+__device__ __forceinline__ double tp_warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+template <typename ST, int TX, int TY, int MINB, int MODE, bool FAST>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* __restrict__ phi,
         double* __restrict__ uout, double* __restrict__ rout, double* __restrict__ phi_new, Seams SM,
         const double* __restrict__ tabs, int lz, const __grid_constant__ CUtensorMap tmap_fin,
-        const __grid_constant__ CUtensorMap tmap_row) {
+        const __grid_constant__ CUtensorMap tmap_row, const double* __restrict__ in0, const double* __restrict__ in1) {
+  constexpr bool FUSED = MODE == MODE_FUSED;
+  constexpr bool PULL = MODE != MODE_INIT;  // the populations of the current state are needed
   static_assert(!FAST || sizeof(ST) == 8, "the TMA pull is for fp64 storage");
+  static_assert(!(FAST && MODE == MODE_INIT), "the push of the initial state uses the per-thread wrap tables");
   using T = GeoTile<ST, TX, TY, FUSED>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
@@ -275,7 +293,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (tx < TY) tma_pull(z0);
+    if (PULL && tx < TY) tma_pull(z0);
   }
   // FAST: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
   // c_ix = -1) are fetched by lanes 0..17 of the row's warp, one 16-byte cp.async each (the aligned pair that holds the
@@ -315,7 +333,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     if (r2 >= 0) cp_async_16(&S.raw[2][0][0] + r2, s2 + r2off);
     cp_async_commit();
   }
-  if (active) prefetch_pull(z0);
+  if (PULL && active) prefetch_pull(z0);
   else cp_async_commit();
 
   // stage raw phi planes z0-2 and z0-1
@@ -352,6 +370,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   int zq2 = pmod(z0 + 1, G.nz);  // wrapped zc + 2, carried (no integer division in the march)
   int sb = 0;                    // element offset of the ring slot of plane zc-1 (slot = it mod NR), carried
   const int zc_last = FUSED ? z1 + 1 : z1;  // FUSED: one more iteration to advect the last plane
+  double dsum[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};  // MODE_DIAG: this thread's partial sums (7) and max |u|
   // One iteration of the march.  STEADY (FAST only): zc in [z0 + 3, z1 - 1], where every phase is active and no plane is
   // the first or the last of the chunk -- the same code with the chunk-boundary conditions resolved at compile time.
   auto iteration = [&](const int zc, auto steady_tag) {
@@ -477,13 +496,19 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     const int z = zc - 1;
     const bool node = STEADY || (z >= z0 && z < z1 && active);
     Moments M;
-    if (node) {
+    if (node && PULL) {
       cp_async_wait_but<1>();
       if (fast) {
         __syncwarp();  // the edge elements were copied by other lanes of this warp
         mbar_wait(&S.fbar, (unsigned)(z - z0) & 1u);
       }
       moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
+    }
+    if (node && !PULL) {  // MODE_INIT: p* given, no momentum, no stress (R15)
+      M.p = __ldg(in0 + (size_t)z * plane + o2off);
+      M.m[0] = M.m[1] = M.m[2] = 0.0;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) M.Pi[j] = 0.0;
     }
     __syncthreads();
     if (adv) {
@@ -519,8 +544,8 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     if (!node) cp_async_commit();
     if (node) {
       // every warp has read its 27 values out of the landing zone (barrier above): refill it for plane z+1
-      if (fast && (STEADY || z + 1 < z1) && tx < TY) tma_pull(z + 1);
-      if (STEADY || z + 1 < z1) prefetch_pull(z + 1);
+      if (PULL && fast && (STEADY || z + 1 < z1) && tx < TY) tma_pull(z + 1);
+      if (PULL && (STEADY || z + 1 < z1)) prefetch_pull(z + 1);
       else cp_async_commit();
       // a3: kappa_c = div n, div q at plane z from the plane sums of z-1, z, z+1
       const double kc = (1.0 / 72.0) * (Pn + (an2 + bn2));
@@ -530,7 +555,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const unsigned k = (unsigned)z * plane + o2off;
       // phi-only part of Eq. 3: r = D lap phi - kappa div q
       if (FUSED) S.e[cj][tid] -= P.kappa * divq;  // (cj was advanced above: slot of plane z = zc-1)
-      else rout[k] = P.D * lapp - P.kappa * divq;
+      else if (MODE == MODE_UNFUSED) rout[k] = P.D * lapp - P.kappa * divq;
 
       // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
       double Fb[3] = {0.0, 0.0, 0.0};
@@ -548,7 +573,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         }
       }
       double A[3], rho;
-      accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, true, A, rho);
+      accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, MODE != MODE_INIT, A, rho);
       const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
       if (FUSED) {
         S.ux[tid] = u[0];
@@ -569,12 +594,46 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         }
         if (!STEADY && z == z0) SM.sz[(2u * blockIdx.z) * plane + o2off] = u[2];
         if (!STEADY && z == z1 - 1) SM.sz[(2u * blockIdx.z + 1u) * plane + o2off] = u[2];
-      } else {
-        uout[k] = u[0];
-        uout[(size_t)G.n + k] = u[1];
-        uout[2 * (size_t)G.n + k] = u[2];
+      } else if (MODE == MODE_UNFUSED || MODE == MODE_MOMENTS) {
+        if (MODE == MODE_UNFUSED || uout) {
+          uout[k] = u[0];
+          uout[(size_t)G.n + k] = u[1];
+          uout[2 * (size_t)G.n + k] = u[2];
+        }
+        if (MODE == MODE_MOMENTS && rout) rout[k] = M.p;
       }
-      collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
+      if (MODE == MODE_FUSED || MODE == MODE_UNFUSED) collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
+      if (MODE == MODE_DIAG) {  // R21: rho |u|^2 / 2, nu a:a / (2 cs4 tau^2), phi, p*, m, max |u|
+        double a6[6];
+        hermite_coeff(M, u, A, a6);
+        const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+        const double aa = a6[0] * a6[0] + a6[1] * a6[1] + a6[2] * a6[2] + 2.0 * (a6[3] * a6[3] + a6[4] * a6[4] + a6[5] * a6[5]);
+        dsum[0] += 0.5 * rho * uu;
+        dsum[1] += P.eps_pref * aa;
+        dsum[2] += phi0;
+        dsum[3] += M.p;
+        dsum[4] += M.m[0];
+        dsum[5] += M.m[1];
+        dsum[6] += M.m[2];
+        dsum[7] = fmax(dsum[7], sqrt(uu));
+      }
+      if (MODE == MODE_INIT) {  // R15: f_i = f_i^eq(p*, u0) - S_i(u0, A)/2, pushed to x - c_i
+        const double u0[3] = {__ldg(in1 + k), __ldg(in1 + (size_t)G.n + k), __ldg(in1 + 2 * (size_t)G.n + k)};
+        const double U[3] = {u0[0] - 0.5 * A[0], u0[1] - 0.5 * A[1], u0[2] - 0.5 * A[2]};
+        double Tt[6];
+        Tt[0] = u0[0] * u0[0] - u0[0] * A[0];
+        Tt[1] = u0[1] * u0[1] - u0[1] * A[1];
+        Tt[2] = u0[2] * u0[2] - u0[2] * A[2];
+        Tt[3] = u0[0] * u0[1] - 0.5 * (u0[0] * A[1] + u0[1] * A[0]);
+        Tt[4] = u0[0] * u0[2] - 0.5 * (u0[0] * A[2] + u0[2] * A[0]);
+        Tt[5] = u0[1] * u0[2] - 0.5 * (u0[1] * A[2] + u0[2] * A[1]);
+        double f[Q];
+        hermite2_populations(M.p, U, Tt, f);
+        ST* slab[3] = {pop_slab(fout, G, wrap_dec(z, G.nz)), pop_slab(fout, G, z), pop_slab(fout, G, wrap_inc(z, G.nz))};
+#pragma unroll
+        for (int i = 0; i < Q; ++i)
+          Pop<ST>::store(slab[1 - cz_of(i)] + ((unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)]), i, f[i]);
+      }
     }
     Pn = fma(4.0, an2, Qn); Qn = an2 - bn2;
     Pq = fma(4.0, aq2, Qq); Qq = aq2 - bq2;
@@ -588,6 +647,28 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     for (; zc <= z1 - 1; ++zc) iteration(zc, std::true_type{});
   }
   for (; zc <= zc_last; ++zc) iteration(zc, std::false_type{});
+  if (MODE == MODE_DIAG) {  // north-star (e): warp shuffle, then one atomic per block and quantity
+    __syncthreads();
+    double* sh = reinterpret_cast<double*>(&S.nq[0][0][0]);  // [8][TY]
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+      const double r = tp_warp_sum(dsum[j]);
+      if (tx == 0) sh[j * TY + ty] = r;
+    }
+    {
+      double v = dsum[7];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+      if (tx == 0) sh[7 * TY + ty] = v;
+    }
+    __syncthreads();
+    if (tid < 8) {
+      double r = sh[tid * TY];
+      for (int w = 1; w < TY; ++w) r = tid < 7 ? r + sh[tid * TY + w] : fmax(r, sh[tid * TY + w]);
+      if (tid < 7) atomicAdd(rout + tid, r);
+      else atomicMax(reinterpret_cast<unsigned long long*>(rout + 7), (unsigned long long)__double_as_longlong(r));  // r >= 0
+    }
+  }
 }
 
 // a8 on the seams of the tile columns of k_lb_tp<FUSED> (R12).  A face is a seam when its two cells
