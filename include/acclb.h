@@ -109,20 +109,20 @@ long long accLB_launch_count(const accLB_ctx* ctx);
 /* Per-kernel device timing.  accLB_profile(ctx, 1) makes every later launch be bracketed by two CUDA events on
  * the context's stream; accLB_profile_read synchronises the stream, adds the elapsed milliseconds and launch
  * counts per kernel kind into ms[k], count[k] for k < min(n, ACCLB_NKERNELS) (HOST pointers) and clears the
- * record.  Kinds (the names are the kernels' own, as an ncu launch list shows them): 0 k_normal, 1 k_lb (the
- * one-node-per-thread fused LB step: single-phase default), 2 k_allen_cahn, 3 k_init, 4 k_moments, 5 k_diagnostics,
- * 6 k_lb_tp (the tiled two-phase step: LB + geometry + advection), 7 k_seam (advective fluxes through the seam faces
- * of its tile columns), 8 k_advect (variant 2 and the Runge-Kutta stages), 9 k_geom_r (D lap phi - kappa div q of a
- * Runge-Kutta stage field).  This is how bench.py measures kernel durations inside the timed region. */
+ * record.  Kinds (the names are the kernels' own, as an ncu launch list shows them): 1 k_lb (the one-node-per-thread fused
+ * LB step of single-phase contexts), 3 k_init, 4 k_moments, 5 k_diagnostics (single-phase kernels, or the tiled kernel
+ * k_lb_tp in its init / moments / diagnostics mode for two-phase contexts), 6 k_lb_tp (the tiled two-phase step: LB +
+ * geometry + advection), 7 k_seam (advective fluxes through the faces between its tile columns), 8 k_advect (variant 1
+ * and the Runge-Kutta stages), 9 k_geom_r (D lap phi - kappa div q of a Runge-Kutta stage field); 0 and 2 are unused.
+ * This is how bench.py measures kernel durations inside the timed region. */
 #define ACCLB_NKERNELS 10
 int accLB_profile(accLB_ctx* ctx, int enable);
 int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
 
-/* Select the kernel variant of the two-phase step: 0 = default (k_lb_tp fused with the advection + k_seam);
- * 1 = one node per thread with stencils straight from global memory (k_normal, k_lb, k_allen_cahn), kept as an
- * in-library cross-check of the tiled path; 2 = round 1's two-kernel form with u and r through HBM (k_lb_tp unfused,
- * k_advect), kept so that bench.py / ncu can compare on identical inputs.  Results are identical
- * to rounding for every variant.  Single-phase contexts have one path.  ACCLB_EINVAL for an unknown variant. */
+/* Select the kernel variant of the forward-Euler two-phase step: 0 = default (k_lb_tp fused with the advection + k_seam);
+ * 1 = the unfused form, u(t) and r through HBM (k_lb_tp unfused + k_advect: the path the SSP-RK3 integrator runs on),
+ * kept so that bench.py / ncu can compare fused and unfused on identical inputs.  Results are
+ * identical to rounding.  Single-phase contexts and phi_integrator = 1 have one path.  ACCLB_EINVAL for an unknown variant. */
 int accLB_set_variant(accLB_ctx* ctx, int variant);
 
 /* Free the context (host memory only; the workspace stays the caller's). */

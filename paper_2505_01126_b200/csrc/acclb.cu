@@ -1,16 +1,15 @@
 // libacclb.so -- kernels and C ABI (include/acclb.h) of the accLB per-time-step lattice update on sm_100a.
 //
 // Written from /root/reference/PAPER.md (arXiv 2505.01126).  One step (rows a1-a8):
-//   k_normal   (two-phase)  n = grad phi / (|grad phi| + 1e-12)                       PAPER.md:L61, L104, R17
-//   k_lb                    pull-stream (a1) -> moments (a2) -> geometry/forces (a3,a4) -> u (a5) ->
-//                           Hermite coefficient (a6) -> regularized reconstruction + aligned store (a7)
-//                                                                                     PAPER.md:L75-92 (Eqs. 4-7)
-//   k_allen_cahn (two-phase) conservative Allen-Cahn, flux-form WENO5 + lattice stencils, forward Euler (a8)
-//                                                                                     PAPER.md:L61-67 (Eq. 3)
-// These three are the one-node-per-thread kernels (single-phase default; two-phase variant 1, kept as an in-library
-// cross-check of the tiled path).  The default two-phase step is the fused k_lb_tp + k_seam (twophase.cuh: shared-memory
-// tiles marching along z, TMA / cp.async staging, u and r never written to HBM); variant 2 is round 1's two-kernel form
-// k_lb_tp<unfused> + k_advect, kept for A/B measurements.
+//   single-phase   k_lb: pull-stream (a1) -> moments (a2) -> body force (a4) -> u (a5) -> Hermite coefficient (a6) ->
+//                  regularized reconstruction + aligned store (a7), one node per thread           PAPER.md:L75-92 (Eqs. 4-7)
+//   two-phase      k_lb_tp<MODE_FUSED> + k_seam (twophase.cuh): the same plus phase geometry, forces (a3, a4) and the
+//                  conservative Allen-Cahn update (a8) on shared-memory tiles marching along z, TMA / cp.async staging;
+//                  u and r never written to HBM                                        PAPER.md:L61-67 (Eq. 3), L100-104 (Eq. 8)
+//                  phi_integrator = 1 (SSP-RK3, R32): k_lb_tp<MODE_UNFUSED> + k_advect stages + k_geom_r (phase_rk.cuh);
+//                  variant 1 = the forward-Euler form of that unfused path (k_lb_tp<MODE_UNFUSED> + k_advect), kept so that
+//                  bench.py / ncu can compare fused and unfused on identical inputs.
+//   init, moments, diagnostics of a two-phase context are modes of the same tiled kernel.
 // State: post-collision, not yet streamed populations f*_i(x) in SoA [z][i][y][x], double-buffered (A/B), so the
 // pull f_i(x,t) = f*_i(x - c_i, t-1) reads shifted rows and every store is aligned; phi double-buffered.
 // No CPU fallback, no library kernels: everything the path computes runs in the kernels of this file.
@@ -147,33 +146,17 @@ __device__ __forceinline__ void accel_from_geometry(const KP& P, const Moments& 
   accel_from_gc(P, M, g, -P.sig15w * kc * gn, phi0, Fb, with_visc, A, rho);
 }
 
-// a3-a5 for the one-node-per-thread kernels: g = grad phi and kappa_c = div n by the lattice stencils
-// straight from global memory (phi, and the normal field written by k_normal), then the force.
-template <bool TWO_PHASE>
-__device__ __forceinline__ void node_accel(const KP& P, const double* __restrict__ phi, const double* __restrict__ nrm,
-                                           const double* __restrict__ tabs, const Nbr& nb, int x, int y, int z,
-                                           const Moments& M, bool with_visc, double (&A)[3], double& rho) {
+// a4-a5 for the one-node-per-thread (single-phase) kernels: rho == 1, A = F^b (+ the uniform (1 - rho_ref) g, R31).
+__device__ __forceinline__ void node_accel(const KP& P, const double* __restrict__ tabs, int x, int y, int z, double (&A)[3],
+                                           double& rho) {
   double Fb[3];
   body_force(P, tabs, x, y, z, Fb);
-  if (!TWO_PHASE) {
-    rho = 1.0;
-    A[0] = Fb[0]; A[1] = Fb[1]; A[2] = Fb[2];
-    if (P.buoyant) {  // single component: the uniform acceleration (1 - rho_ref) g (R31)
-      const double dr = 1.0 - P.rho_ref;
-      A[0] += dr * P.grav[0]; A[1] += dr * P.grav[1]; A[2] += dr * P.grav[2];
-    }
-    return;
+  rho = 1.0;
+  A[0] = Fb[0]; A[1] = Fb[1]; A[2] = Fb[2];
+  if (P.buoyant) {
+    const double dr = 1.0 - P.rho_ref;
+    A[0] += dr * P.grav[0]; A[1] += dr * P.grav[1]; A[2] += dr * P.grav[2];
   }
-  const unsigned n = P.G.n;
-  double g[3];
-  g[0] = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
-  g[1] = lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
-  g[2] = lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(phi + nb.at(dz, dy, dx)); });
-  const double kc = lattice_derivative<0>([&](int dz, int dy, int dx) { return __ldg(nrm + nb.at(dz, dy, dx)); }) +
-                    lattice_derivative<1>([&](int dz, int dy, int dx) { return __ldg(nrm + n + nb.at(dz, dy, dx)); }) +
-                    lattice_derivative<2>([&](int dz, int dy, int dx) { return __ldg(nrm + 2u * n + nb.at(dz, dy, dx)); });
-  const double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
-  accel_from_geometry(P, M, g, gn, kc, __ldg(phi + nb.at(0, 0, 0)), Fb, with_visc, A, rho);
 }
 
 // a6: a_ab = sum_i (f_i - f_i^eq + S_i/2) H_i,ab (Eq. 7) in closed form (O5'):
@@ -217,33 +200,13 @@ __device__ __forceinline__ void collide_store(const KP& P, const Moments& M, con
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
+// The single-phase kernels: one node per thread, scalar 64-bit accesses (at the measured copy bandwidth, DESIGN.md
+// section 7).  Two-phase contexts run the tiled kernel of twophase.cuh in all of its modes.
 
-// Interface normal n = g / (|g| + 1e-12), g = grad phi by the lattice stencil.   PAPER.md:L61, L104; R17
-__global__ void __launch_bounds__(256) k_normal(KP P, const double* __restrict__ phi, double* __restrict__ nrm) {
-  unsigned k; int x, y, z;
-  if (!node_of_thread(P.G, k, x, y, z)) return;
-  Nbr nb;
-  make_nbr(P.G, x, y, z, nb);
-  double v[3][3][3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int b = 0; b < 3; ++b)
-#pragma unroll
-      for (int c = 0; c < 3; ++c) v[a][b][c] = __ldg(phi + nb.row[a][b] + nb.x[c]);
-  double g[3];
-  gradient27(v, g);
-  const double inv = 1.0 / (sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]) + 1e-12);
-  nrm[k] = g[0] * inv;
-  nrm[P.G.n + k] = g[1] * inv;
-  nrm[2u * P.G.n + k] = g[2] * inv;
-}
-
-// The fused LB step, one node per thread (variant 1: scalar 64-bit accesses).
-template <typename ST, bool TWO_PHASE>
+// The fused LB step.
+template <typename ST>
 __global__ void __launch_bounds__(128) k_lb(KP P, const ST* __restrict__ fin, ST* __restrict__ fout,
-                                            const double* __restrict__ phi, const double* __restrict__ nrm,
-                                            double* __restrict__ uout, const double* __restrict__ tabs) {
+                                            const double* __restrict__ tabs) {
   unsigned k; int x, y, z;
   if (!node_of_thread(P.G, k, x, y, z)) return;
   Nbr nb;
@@ -253,91 +216,24 @@ __global__ void __launch_bounds__(128) k_lb(KP P, const ST* __restrict__ fin, ST
   Moments M;
   moments_of(f, M);
   double A[3], rho;
-  node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, true, A, rho);
+  node_accel(P, tabs, x, y, z, A, rho);
   const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
-  if (TWO_PHASE) {
-    uout[k] = u[0];
-    uout[P.G.n + k] = u[1];
-    uout[2u * P.G.n + k] = u[2];
-  }
   const unsigned plane = (unsigned)P.G.nx * (unsigned)P.G.ny;
   collide_store<ST>(P, M, u, A, f, pop_slab(fout, P.G, z) + (nb.yr[1] + (unsigned)x), plane);
 }
 
-// a8: conservative Allen-Cahn update (Eq. 3), forward Euler (R13):
-//   phi+ = phi - sum_e (Phi_e(x) - Phi_e(x - e)) + D lap phi - kappa div(phi (1 - phi) n),
-//   Phi_e = u_f WENO5(phi) in flux form (R12), lap / div by the lattice stencils.
-__global__ void __launch_bounds__(128) k_allen_cahn(KP P, const double* __restrict__ phi, const double* __restrict__ nrm,
-                                                    const double* __restrict__ u, double* __restrict__ phi_new) {
-  unsigned k; int x, y, z;
-  if (!node_of_thread(P.G, k, x, y, z)) return;
-  const Grid& G = P.G;
-  Nbr nb;
-  make_nbr(G, x, y, z, nb);
-  const unsigned n = G.n;
-  double v[3][3][3], pq[3][3][3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int b = 0; b < 3; ++b)
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        const double ph = __ldg(phi + nb.row[a][b] + nb.x[c]);
-        v[a][b][c] = ph;
-        pq[a][b][c] = ph * (1.0 - ph);
-      }
-  const double lap = laplacian27(v);
-  const double divq =
-      lattice_derivative<0>([&](int dz, int dy, int dx) { return pq[dz + 1][dy + 1][dx + 1] * __ldg(nrm + nb.at(dz, dy, dx)); }) +
-      lattice_derivative<1>([&](int dz, int dy, int dx) { return pq[dz + 1][dy + 1][dx + 1] * __ldg(nrm + n + nb.at(dz, dy, dx)); }) +
-      lattice_derivative<2>([&](int dz, int dy, int dx) { return pq[dz + 1][dy + 1][dx + 1] * __ldg(nrm + 2u * n + nb.at(dz, dy, dx)); });
-
-  double adv = 0.0;
-  {  // x faces
-    const unsigned r = nb.row[1][1];
-    const double pm3 = __ldg(phi + r + wrap_add(x, -3, G.nx)), pm2 = __ldg(phi + r + wrap_add(x, -2, G.nx));
-    const double pp2 = __ldg(phi + r + wrap_add(x, 2, G.nx)), pp3 = __ldg(phi + r + wrap_add(x, 3, G.nx));
-    const double um = __ldg(u + nb.at(0, 0, -1)), u0 = __ldg(u + k), up = __ldg(u + nb.at(0, 0, 1));
-    adv += face_flux(u0, up, pm2, v[1][1][0], v[1][1][1], v[1][1][2], pp2, pp3) -
-           face_flux(um, u0, pm3, pm2, v[1][1][0], v[1][1][1], v[1][1][2], pp2);
-  }
-  {  // y faces
-    const unsigned rz = (unsigned)z * (unsigned)G.ny;
-    auto at = [&](int kk) { return (rz + (unsigned)wrap_add(y, kk, G.ny)) * (unsigned)G.nx + (unsigned)x; };
-    const double pm3 = __ldg(phi + at(-3)), pm2 = __ldg(phi + at(-2)), pp2 = __ldg(phi + at(2)), pp3 = __ldg(phi + at(3));
-    const double* uy = u + n;
-    const double um = __ldg(uy + nb.at(0, -1, 0)), u0 = __ldg(uy + k), up = __ldg(uy + nb.at(0, 1, 0));
-    adv += face_flux(u0, up, pm2, v[1][0][1], v[1][1][1], v[1][2][1], pp2, pp3) -
-           face_flux(um, u0, pm3, pm2, v[1][0][1], v[1][1][1], v[1][2][1], pp2);
-  }
-  {  // z faces
-    auto at = [&](int kk) { return ((unsigned)wrap_add(z, kk, G.nz) * (unsigned)G.ny + (unsigned)y) * (unsigned)G.nx + (unsigned)x; };
-    const double pm3 = __ldg(phi + at(-3)), pm2 = __ldg(phi + at(-2)), pp2 = __ldg(phi + at(2)), pp3 = __ldg(phi + at(3));
-    const double* uz = u + 2u * n;
-    const double um = __ldg(uz + nb.at(-1, 0, 0)), u0 = __ldg(uz + k), up = __ldg(uz + nb.at(1, 0, 0));
-    adv += face_flux(u0, up, pm2, v[0][1][1], v[1][1][1], v[2][1][1], pp2, pp3) -
-           face_flux(um, u0, pm3, pm2, v[0][1][1], v[1][1][1], v[2][1][1], pp2);
-  }
-  phi_new[k] = v[1][1][1] + (-adv + P.D * lap - P.kappa * divq);
-}
-
-// Initial populations (R15): f_i(x,0) = f_i^eq(p*,u0) - S_i(u0,A)/2 with A from F^s + F^p + F^b (F^nu := 0),
-// written "pushed" to x - c_i so that the first pull returns them at x.
-template <typename ST, bool TWO_PHASE>
+// Initial populations (R15): f_i(x,0) = f_i^eq(p*,u0) - S_i(u0,A)/2 with A = F^b (+ F^g), written "pushed" to x - c_i so
+// that the first pull returns them at x.
+template <typename ST>
 __global__ void __launch_bounds__(128) k_init(KP P, const double* __restrict__ rho_in, const double* __restrict__ u_in,
-                                              const double* __restrict__ phi, const double* __restrict__ nrm,
                                               const double* __restrict__ tabs, ST* __restrict__ fout) {
   unsigned k; int x, y, z;
   if (!node_of_thread(P.G, k, x, y, z)) return;
   Nbr nb;
   make_nbr(P.G, x, y, z, nb);
-  Moments M;
-  M.p = rho_in[k];
-  M.m[0] = M.m[1] = M.m[2] = 0.0;
-#pragma unroll
-  for (int j = 0; j < 6; ++j) M.Pi[j] = 0.0;
   double A[3], rho;
-  node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, false, A, rho);
+  node_accel(P, tabs, x, y, z, A, rho);
+  const double p = rho_in[k];
   const double u[3] = {u_in[k], u_in[P.G.n + k], u_in[2u * P.G.n + k]};
   const double U[3] = {u[0] - 0.5 * A[0], u[1] - 0.5 * A[1], u[2] - 0.5 * A[2]};
   double T[6];
@@ -348,7 +244,7 @@ __global__ void __launch_bounds__(128) k_init(KP P, const double* __restrict__ r
   T[4] = u[0] * u[2] - 0.5 * (u[0] * A[2] + u[2] * A[0]);
   T[5] = u[1] * u[2] - 0.5 * (u[1] * A[2] + u[2] * A[1]);
   double f[Q];
-  hermite2_populations(M.p, U, T, f);
+  hermite2_populations(p, U, T, f);
 #pragma unroll
   for (int i = 0; i < Q; ++i)
     Pop<ST>::store(pop_slab(fout, P.G, nb.z[1 - cz_of(i)]) +
@@ -357,9 +253,8 @@ __global__ void __launch_bounds__(128) k_init(KP P, const double* __restrict__ r
 }
 
 // a9: (p*, u) of the current state; the state is unchanged.
-template <typename ST, bool TWO_PHASE>
-__global__ void __launch_bounds__(128) k_moments(KP P, const ST* __restrict__ fin, const double* __restrict__ phi,
-                                                 const double* __restrict__ nrm, const double* __restrict__ tabs,
+template <typename ST>
+__global__ void __launch_bounds__(128) k_moments(KP P, const ST* __restrict__ fin, const double* __restrict__ tabs,
                                                  double* __restrict__ rho_out, double* __restrict__ u_out) {
   unsigned k; int x, y, z;
   if (!node_of_thread(P.G, k, x, y, z)) return;
@@ -370,7 +265,7 @@ __global__ void __launch_bounds__(128) k_moments(KP P, const ST* __restrict__ fi
   Moments M;
   moments_of(f, M);
   double A[3], rho;
-  node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, true, A, rho);
+  node_accel(P, tabs, x, y, z, A, rho);
   if (rho_out) rho_out[k] = M.p;
   if (u_out) {
     u_out[k] = M.m[0] + 0.5 * A[0];
@@ -379,8 +274,8 @@ __global__ void __launch_bounds__(128) k_moments(KP P, const ST* __restrict__ fi
   }
 }
 
-// a9: diagnostics (R21).  acc[0..6] += sum (rho |u|^2/2, eps, phi, p*, m_x, m_y, m_z); acc[7] = max |u| (as ordered
-// bits).  Grid-stride; per-thread partials -> warp shuffle -> one atomic per block and quantity.
+// a9: diagnostics (R21).  acc[0..6] += sum (|u|^2/2, eps, 0, p*, m_x, m_y, m_z); acc[7] = max |u| (as ordered bits).
+// Grid-stride; per-thread partials -> warp shuffle -> one atomic per block and quantity.
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -394,10 +289,8 @@ __device__ __forceinline__ double warp_max(double v) {
 
 constexpr int DIAG_THREADS = 128;
 
-template <typename ST, bool TWO_PHASE>
+template <typename ST>
 __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __restrict__ fin,
-                                                              const double* __restrict__ phi,
-                                                              const double* __restrict__ nrm,
                                                               const double* __restrict__ tabs, double* __restrict__ acc) {
   double s[7] = {0, 0, 0, 0, 0, 0, 0};
   double umax = 0.0;
@@ -413,7 +306,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
     Moments M;
     moments_of(f, M);
     double A[3], rho;
-    node_accel<TWO_PHASE>(P, phi, nrm, tabs, nb, x, y, z, M, true, A, rho);
+    node_accel(P, tabs, x, y, z, A, rho);
     const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};
     double a[6];
     hermite_coeff(M, u, A, a);
@@ -421,7 +314,6 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
     const double aa = a[0] * a[0] + a[1] * a[1] + a[2] * a[2] + 2.0 * (a[3] * a[3] + a[4] * a[4] + a[5] * a[5]);
     s[0] += 0.5 * rho * uu;
     s[1] += P.eps_pref * aa;
-    if (TWO_PHASE) s[2] += __ldg(phi + k);
     s[3] += M.p;
     s[4] += M.m[0];
     s[5] += M.m[1];
@@ -469,7 +361,6 @@ struct accLB_ctx {
   double* u;
   double* r;    // D lap phi - kappa div q of the current step (k_lb_tp -> k_advect)
   double* phis; // RK3 only: the second stage field
-  double* nrm;
   double* tabs;
   double* acc;
   CUtensorMap tmap[2];      // populations A / B as rank-3 tensors (x, y, z * 27 + i) for the TMA pull of k_lb_tp<FAST>,
@@ -546,7 +437,7 @@ struct LaunchScope {
     }
   }
 };
-enum { KIND_NORMAL = 0, KIND_LB = 1, KIND_AC = 2, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_LB_TP = 6,
+enum { KIND_LB = 1, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_LB_TP = 6,
        KIND_SEAM = 7, KIND_ADVECT = 8, KIND_GEOM = 9 };
 
 static thread_local char g_err[512] = "";
@@ -596,7 +487,7 @@ static int planes_per_block(int nx, int ny, int nz, int tx, int ty) {
 }
 
 struct Carve {
-  size_t f, phi, u, r, nrm, tabs, acc, sx, sy, sz, phis, stage, total;
+  size_t f, phi, u, r, tabs, acc, sx, sy, sz, phis, stage, total;
 };
 static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   const size_t n = (size_t)nx * ny * nz;
@@ -605,7 +496,6 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   c.phi = p->two_phase ? align256(n * 8) : 0;
   c.u = p->two_phase ? align256(3 * n * 8) : 0;
   c.r = p->two_phase ? align256(n * 8) : 0;
-  c.nrm = p->two_phase ? align256(3 * n * 8) : 0;
   c.tabs = align256((size_t)2 * (nx + ny + nz) * 8);
   c.acc = align256(16 * 8);
   const size_t ntx = (nx + LBT_TX - 1) / LBT_TX, nty = (ny + LBT_TY - 1) / LBT_TY;
@@ -616,7 +506,7 @@ static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   c.sz = p->two_phase ? align256(2 * nchunk * (size_t)ny * nx * 8) : 0;
   c.phis = p->two_phase && p->phi_integrator == 1 ? align256(n * 8) : 0;
   c.stage = p->host_staging ? align256(5 * n * 8) : 0;
-  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.nrm + c.tabs + c.acc + c.sx + c.sy + c.sz + c.phis + c.stage;
+  c.total = 2 * c.f + 2 * c.phi + c.u + c.r + c.tabs + c.acc + c.sx + c.sy + c.sz + c.phis + c.stage;
   return c;
 }
 
@@ -777,7 +667,6 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   s->phi[1] = p->two_phase ? (double*)w : nullptr; w += c.phi;
   s->u = p->two_phase ? (double*)w : nullptr; w += c.u;
   s->r = p->two_phase ? (double*)w : nullptr; w += c.r;
-  s->nrm = p->two_phase ? (double*)w : nullptr; w += c.nrm;
   s->tabs = (double*)w; w += c.tabs;
   s->acc = (double*)w; w += c.acc;
   s->seams.sx = p->two_phase ? (double*)w : nullptr; w += c.sx;
@@ -833,15 +722,6 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   return ACCLB_OK;
 }
 
-static int launch_normal(accLB_ctx* s) {
-  {
-    LaunchScope ls(s, KIND_NORMAL);
-    k_normal<<<blocks_for(s->n, 256), 256, 0, s->stream>>>(s->kp, s->phi[s->cur], s->nrm);
-  }
-  CK(cudaGetLastError());
-  return ACCLB_OK;
-}
-
 int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* phi) {
   if (!s || !rho || !u) return fail(ACCLB_EINVAL, "accLB_init: NULL argument");
   if (s->prm.two_phase && !phi) return fail(ACCLB_EINVAL, "accLB_init: phi is NULL for a two-phase context");
@@ -857,9 +737,9 @@ int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* p
   } else {
     LaunchScope ls(s, KIND_INIT);
     if (s->prm.store_fp32)
-      k_init<float, false><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, nullptr, nullptr, s->tabs, (float*)s->f[0]);
+      k_init<float><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, s->tabs, (float*)s->f[0]);
     else
-      k_init<double, false><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, nullptr, nullptr, s->tabs, (double*)s->f[0]);
+      k_init<double><<<nb, 128, 0, s->stream>>>(s->kp, rho, u, s->tabs, (double*)s->f[0]);
   }
   CK(cudaGetLastError());
   return ACCLB_OK;
@@ -886,33 +766,18 @@ int accLB_step(accLB_ctx* s, int nsteps) {
       if (r) return r;
       r = launch_seam(s, c, d);
       if (r) return r;
-    } else if (s->prm.two_phase && s->variant == 2) {
-      // variant 2: round 1's two-kernel form, u and r through HBM (k_lb_tp<unfused>, k_advect)
+    } else if (s->prm.two_phase) {
+      // variant 1: the forward-Euler form of the unfused path, u and r through HBM (k_lb_tp<MODE_UNFUSED>, k_advect)
       int r = launch_lb_tp_any<MODE_UNFUSED>(s, c, d);
       if (r) return r;
       r = launch_advect(s, s->phi[c], s->phi[d]);
       if (r) return r;
-    } else if (s->prm.two_phase) {
-      // variant 1: one node per thread, stencils straight from global memory (k_normal, k_lb, k_allen_cahn)
-      int r = launch_normal(s);
-      if (r) return r;
-      {
-        LaunchScope ls(s, KIND_LB);
-        if (s->prm.store_fp32)
-          k_lb<float, true><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], (float*)s->f[d], s->phi[c], s->nrm, s->u, s->tabs);
-        else
-          k_lb<double, true><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], (double*)s->f[d], s->phi[c], s->nrm, s->u, s->tabs);
-      }
-      {
-        LaunchScope ls(s, KIND_AC);
-        k_allen_cahn<<<nb, 128, 0, s->stream>>>(s->kp, s->phi[c], s->nrm, s->u, s->phi[d]);
-      }
     } else {
       LaunchScope ls(s, KIND_LB);
       if (s->prm.store_fp32)
-        k_lb<float, false><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], (float*)s->f[d], nullptr, nullptr, nullptr, s->tabs);
+        k_lb<float><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], (float*)s->f[d], s->tabs);
       else
-        k_lb<double, false><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], (double*)s->f[d], nullptr, nullptr, nullptr, s->tabs);
+        k_lb<double><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], (double*)s->f[d], s->tabs);
     }
     s->cur = d;
     s->step += 1;
@@ -935,9 +800,9 @@ int accLB_moments(accLB_ctx* s, double* rho, double* u, double* phi) {
   } else {
     LaunchScope ls(s, KIND_MOMENTS);
     if (s->prm.store_fp32)
-      k_moments<float, false><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], nullptr, nullptr, s->tabs, rho, u);
+      k_moments<float><<<nb, 128, 0, s->stream>>>(s->kp, (const float*)s->f[c], s->tabs, rho, u);
     else
-      k_moments<double, false><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], nullptr, nullptr, s->tabs, rho, u);
+      k_moments<double><<<nb, 128, 0, s->stream>>>(s->kp, (const double*)s->f[c], s->tabs, rho, u);
   }
   CK(cudaGetLastError());
   return ACCLB_OK;
@@ -957,9 +822,9 @@ int accLB_diagnostics(accLB_ctx* s, double* out, int n_out) {
   } else {
     LaunchScope ls(s, KIND_DIAG);
     if (s->prm.store_fp32)
-      k_diagnostics<float, false><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const float*)s->f[c], nullptr, nullptr, s->tabs, s->acc);
+      k_diagnostics<float><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const float*)s->f[c], s->tabs, s->acc);
     else
-      k_diagnostics<double, false><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const double*)s->f[c], nullptr, nullptr, s->tabs, s->acc);
+      k_diagnostics<double><<<nb, DIAG_THREADS, 0, s->stream>>>(s->kp, (const double*)s->f[c], s->tabs, s->acc);
   }
   CK(cudaGetLastError());
   double h[8];
@@ -1016,7 +881,7 @@ long long accLB_launch_count(const accLB_ctx* s) { return s ? s->launches : 0; }
 
 int accLB_set_variant(accLB_ctx* s, int variant) {
   if (!s) return fail(ACCLB_EINVAL, "accLB_set_variant: NULL context");
-  if (variant < 0 || variant > 2) return fail(ACCLB_EINVAL, "accLB_set_variant: unknown variant %d", variant);
+  if (variant < 0 || variant > 1) return fail(ACCLB_EINVAL, "accLB_set_variant: unknown variant %d", variant);
   s->variant = variant;
   return ACCLB_OK;
 }

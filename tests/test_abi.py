@@ -48,8 +48,11 @@ def test_workspace_bytes(lib):
     # seam strips of the 32 x 8 tile columns: u_x on 2 columns per tile column, u_y on 2 rows per tile row, u_z on 2
     # planes per z chunk (32^3: 1 tile column, 4 tile rows, chunks of 8 planes)
     seams = a256(32 * 32 * 2 * 1 * 8) + a256(32 * 2 * 4 * 32 * 8) + a256(2 * 4 * 32 * 32 * 8)
-    assert binding.workspace_bytes(32, 32, 32, p) == (2 * a256(27 * n * 8) + 3 * a256(n * 8) + 2 * a256(3 * n * 8) + small
+    # two population buffers, phi A / B, r, u (the unfused paths), seam strips, host staging
+    assert binding.workspace_bytes(32, 32, 32, p) == (2 * a256(27 * n * 8) + 3 * a256(n * 8) + a256(3 * n * 8) + small
                                                       + seams + a256(5 * n * 8))
+    p_rk = binding.make_params(tau=0.8, two_phase=1, mobility=0.05, sigma=0.01, host_staging=1, phi_rk3=1)
+    assert binding.workspace_bytes(32, 32, 32, p_rk) == binding.workspace_bytes(32, 32, 32, p) + a256(n * 8)  # stage field
     # 512^3 two-phase fp64 fits one B200 (180 GB) with room to spare
     p = binding.make_params(tau=0.505, two_phase=1, mobility=0.05, sigma=0.02)
     assert 60e9 < binding.workspace_bytes(512, 512, 512, p) < 70e9

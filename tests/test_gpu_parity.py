@@ -195,7 +195,7 @@ def test_two_phase_ragged_box_ratio10_with_forcing(acclb, shape):
     assert abs(dg["sum_phi"] - do["sum_phi"]) <= 1e-12 * do["sum_phi"]
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("shape", [(4, 4, 4), (6, 4, 8), (8, 12, 4)])
 def test_two_phase_minimum_size_boxes(acclb, shape, variant):
     """The smallest boxes the ABI admits (nx, ny, nz >= 4): every tile wraps onto itself several times, the WENO5
@@ -309,26 +309,21 @@ def test_launch_count_and_errors(acclb):
     c0 = sim2.launch_count
     sim2.step(4)
     assert sim2.launch_count - c0 == 8         # LB + geometry + advection fused on tiles, then the seam faces (one launch)
-    sim2.set_variant(2)
-    c0 = sim2.launch_count
-    sim2.step(4)
-    assert sim2.launch_count - c0 == 8         # variant 2: round 1's two-kernel form (u, r through HBM)
     sim2.set_variant(1)
     c0 = sim2.launch_count
     sim2.step(4)
-    assert sim2.launch_count - c0 == 12        # variant 1: normal + LB + Allen-Cahn
+    assert sim2.launch_count - c0 == 8         # variant 1: the unfused two-kernel form (u, r through HBM)
     with pytest.raises(acclb.AccLBError):
         sim.step(-1)
     with pytest.raises(acclb.AccLBError):
         acclb.AccLB(31, 32, 32, tau=0.8)
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1])
 @pytest.mark.parametrize("ratio", [1.0, 10.0])
 def test_variant_kernels_match_oracle_and_default(acclb, ratio, variant):
-    """Variant 1 (one node per thread, stencils from global memory), variant 2 (tiled, u and r through HBM) and the
-    default fused path agree with the oracle and with each other to rounding; switching variants in mid-run is
-    allowed."""
+    """Variant 1 (tiled, u and r through HBM, separate flux kernel) and the default fused path agree with the oracle and
+    with each other to rounding; switching variants in mid-run is allowed."""
     cfg = wl.make_config("droplet", n=40, density_ratio=ratio)
     a, b, o = gpu_sim(acclb, cfg), gpu_sim(acclb, cfg), cpu_sim(cfg)
     b.set_variant(variant)
