@@ -131,6 +131,29 @@ int accLB_destroy(accLB_ctx* ctx);
 /* Text of the last error on this thread ("" if none).  The pointer stays valid until the next call. */
 const char* accLB_last_error(void);
 
+/* ---- On-device turbulence statistics of a velocity field.  Context-free:
+ * u is a DEVICE pointer to [3][nz][ny][nx] fp64 (e.g. the u of accLB_moments), results go to HOST pointers, `scratch` is a
+ * small caller-owned DEVICE block (8-byte aligned) for the accumulators; the calls synchronise `stream`.
+ *
+ * accLB_stats_increments: longitudinal structure functions, for each separation r[j] >= 0 (HOST array):
+ *   out[3 j + p - 2] = S_p(r_j) = < (u_a(x + r e_a) - u_a(x))^p >, p = 2, 3, 4, averaged over all nodes and the three
+ *   axes a (periodic).  The longitudinal gradient of PAPER.md:L183, taken as the central difference, has the moments
+ *   S_p(2) / 2^p: skewness S_3(2) / S_2(2)^{3/2}, flatness S_4(2) / S_2(2)^2.  scratch >= 3 nr doubles.
+ * accLB_stats_pdf: histogram of d / scale, d the same increments at separation r (r = 2, scale = 2 rms: the gradient PDF of
+ *   PAPER.md Fig. 3a; any r: the increment PDFs of Fig. 6), nbins <= 1024 equal bins on [lo, hi); values outside go to
+ *   the first / last bin.  counts: HOST, nbins entries, sum = 3 nx ny nz.  scratch >= nbins 8-byte counters.
+ * accLB_stats_spectrum: shell sums of a real-to-complex transform (Fig. 2, 5): uhat is a DEVICE pointer to
+ *   [ncomp][nz][ny][nx/2 + 1] complex fp64 (re, im interleaved), the UNNORMALISED transform of ncomp real fields (the FFT
+ *   is the caller's library call); E[k] = sum over the modes with round(|k|) = k of |uhat|^2 / (2 N^2), the conjugate
+ *   half counted, k = 0 .. nshell - 1, so that sum_k E[k] = < f.f > / 2 when nshell covers all modes.  scratch >= nshell
+ *   doubles. */
+int accLB_stats_increments(const double* u, int nx, int ny, int nz, const int* r, int nr, double* out, void* scratch,
+                           size_t scratch_bytes, int device, void* stream);
+int accLB_stats_pdf(const double* u, int nx, int ny, int nz, int r, double scale, double lo, double hi, int nbins,
+                    unsigned long long* counts, void* scratch, size_t scratch_bytes, int device, void* stream);
+int accLB_stats_spectrum(const double* uhat, int nx, int ny, int nz, int ncomp, int nshell, double* E, void* scratch,
+                         size_t scratch_bytes, int device, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ ERRORS = {0: "ACCLB_OK", -1: "ACCLB_EINVAL", -2: "ACCLB_EWORKSPACE", -3: "ACCLB_
 SYMBOLS = ("accLB_workspace_bytes", "accLB_create", "accLB_init", "accLB_step", "accLB_moments",
            "accLB_diagnostics", "accLB_run_host", "accLB_launch_count", "accLB_profile",
            "accLB_profile_read", "accLB_set_variant", "accLB_destroy",
-           "accLB_last_error")
+           "accLB_last_error", "accLB_stats_increments", "accLB_stats_pdf", "accLB_stats_spectrum")
 
 
 class Params(C.Structure):
@@ -74,6 +74,12 @@ def load():
     L.accLB_set_variant.argtypes = [C.c_void_p, C.c_int]
     L.accLB_destroy.argtypes = [C.c_void_p]
     L.accLB_last_error.restype = C.c_char_p
+    L.accLB_stats_increments.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_double), _dp,
+                                         C.c_size_t, C.c_int, C.c_void_p]
+    L.accLB_stats_pdf.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
+                                  C.POINTER(C.c_ulonglong), _dp, C.c_size_t, C.c_int, C.c_void_p]
+    L.accLB_stats_spectrum.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), _dp, C.c_size_t,
+                                       C.c_int, C.c_void_p]
     _lib = L
     return L
 
@@ -194,3 +200,49 @@ class AccLB:
     @property
     def launch_count(self):
         return int(load().accLB_launch_count(self._h))
+
+
+# ---------------------------------------------------------------------------------------- turbulence statistics (8(f) #4)
+def _stats_common(t, ndim):
+    import torch
+    assert t.is_cuda and t.is_contiguous() and t.dim() == ndim, (t.device, tuple(t.shape))
+    dev = t.device
+    return torch, dev, torch.cuda.current_stream(dev).cuda_stream
+
+
+def stats_increments(u, separations):
+    """S_p(r), p = 2, 3, 4, of the longitudinal velocity increments of u [3][nz][ny][nx] (CUDA fp64): array [nr][3]."""
+    torch, dev, stream = _stats_common(u, 4)
+    assert u.dtype == torch.float64 and u.shape[0] == 3
+    _, nz, ny, nx = u.shape
+    nr = len(separations)
+    r = (C.c_int * nr)(*[int(v) for v in separations])
+    out = (C.c_double * (3 * nr))()
+    scratch = torch.empty(3 * nr, dtype=torch.float64, device=dev)
+    _check(load().accLB_stats_increments(u.data_ptr(), nx, ny, nz, r, nr, out, scratch.data_ptr(), scratch.numel() * 8,
+                                         dev.index or 0, stream))
+    return [[out[3 * j + p] for p in range(3)] for j in range(nr)]
+
+
+def stats_pdf(u, r, scale, lo, hi, nbins):
+    """Histogram (nbins counts) of the longitudinal increments at separation r, divided by scale, on [lo, hi)."""
+    torch, dev, stream = _stats_common(u, 4)
+    assert u.dtype == torch.float64 and u.shape[0] == 3
+    _, nz, ny, nx = u.shape
+    counts = (C.c_ulonglong * nbins)()
+    scratch = torch.empty(nbins, dtype=torch.int64, device=dev)
+    _check(load().accLB_stats_pdf(u.data_ptr(), nx, ny, nz, int(r), float(scale), float(lo), float(hi), int(nbins), counts,
+                                  scratch.data_ptr(), scratch.numel() * 8, dev.index or 0, stream))
+    return list(counts)
+
+
+def stats_spectrum(uhat, nx, nshell):
+    """Shell sums E[k] of uhat = rfftn of ncomp real fields, [ncomp][nz][ny][nx/2+1] complex128 (the caller's FFT)."""
+    torch, dev, stream = _stats_common(uhat, 4)
+    assert uhat.dtype == torch.complex128 and uhat.shape[3] == nx // 2 + 1
+    ncomp, nz, ny, _ = uhat.shape
+    E = (C.c_double * nshell)()
+    scratch = torch.empty(nshell, dtype=torch.float64, device=dev)
+    _check(load().accLB_stats_spectrum(uhat.data_ptr(), nx, ny, nz, ncomp, int(nshell), E, scratch.data_ptr(),
+                                       scratch.numel() * 8, dev.index or 0, stream))
+    return list(E)

@@ -345,6 +345,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
 
 #include "twophase.cuh"
 #include "phase_rk.cuh"
+#include "stats.cuh"
 
 // ================================================================================================== host / ABI
 using namespace acclb;
@@ -922,5 +923,74 @@ int accLB_destroy(accLB_ctx* s) {
 }
 
 const char* accLB_last_error(void) { return g_err; }
+
+// ---------------------------------------------------------------------------------------- turbulence statistics (8(f) #4)
+static bool stats_args(const void* u, int nx, int ny, int nz, const void* scratch) {
+  return u && scratch && nx >= 1 && ny >= 1 && nz >= 1 && (double)nx * ny * nz < 2147483648.0;
+}
+static unsigned stats_blocks(size_t n) {
+  const size_t b = (n + STATS_THREADS - 1) / STATS_THREADS, cap = 148 * 8;
+  return (unsigned)(b < cap ? b : cap);
+}
+
+int accLB_stats_increments(const double* u, int nx, int ny, int nz, const int* r, int nr, double* out, void* scratch,
+                           size_t scratch_bytes, int device, void* stream) {
+  if (!stats_args(u, nx, ny, nz, scratch) || !r || !out || nr < 1) return fail(ACCLB_EINVAL, "accLB_stats_increments: bad argument");
+  if (scratch_bytes < (size_t)nr * 3 * sizeof(double) || ((size_t)scratch & 7))
+    return fail(ACCLB_EWORKSPACE, "accLB_stats_increments: scratch of %zu bytes, need %zu", scratch_bytes, (size_t)nr * 3 * sizeof(double));
+  DeviceGuard guard_(device);
+  if (!guard_.ok) return fail(ACCLB_ECUDA, "accLB_stats_increments: cannot select device %d", device);
+  cudaStream_t st = (cudaStream_t)stream;
+  Grid G{nx, ny, nz, (unsigned)((size_t)nx * ny * nz)};
+  double* acc = (double*)scratch;
+  CK(cudaMemsetAsync(acc, 0, (size_t)nr * 3 * sizeof(double), st));
+  for (int j = 0; j < nr; ++j) {
+    if (r[j] < 0) return fail(ACCLB_EINVAL, "accLB_stats_increments: negative separation");
+    k_stats_increments<<<stats_blocks(G.n), STATS_THREADS, 0, st>>>(G, u, r[j], acc + 3 * j);
+  }
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, acc, (size_t)nr * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  const double inv = 1.0 / (3.0 * (double)G.n);
+  for (int j = 0; j < 3 * nr; ++j) out[j] *= inv;
+  return ACCLB_OK;
+}
+
+int accLB_stats_pdf(const double* u, int nx, int ny, int nz, int r, double scale, double lo, double hi, int nbins,
+                    unsigned long long* counts, void* scratch, size_t scratch_bytes, int device, void* stream) {
+  if (!stats_args(u, nx, ny, nz, scratch) || !counts || r < 0 || !(scale > 0.0) || !(hi > lo) || nbins < 1 || nbins > STATS_MAX_BINS)
+    return fail(ACCLB_EINVAL, "accLB_stats_pdf: bad argument (1 <= nbins <= %d, hi > lo, scale > 0)", STATS_MAX_BINS);
+  if (scratch_bytes < (size_t)nbins * sizeof(unsigned long long) || ((size_t)scratch & 7))
+    return fail(ACCLB_EWORKSPACE, "accLB_stats_pdf: scratch too small");
+  DeviceGuard guard_(device);
+  if (!guard_.ok) return fail(ACCLB_ECUDA, "accLB_stats_pdf: cannot select device %d", device);
+  cudaStream_t st = (cudaStream_t)stream;
+  Grid G{nx, ny, nz, (unsigned)((size_t)nx * ny * nz)};
+  unsigned long long* c = (unsigned long long*)scratch;
+  CK(cudaMemsetAsync(c, 0, (size_t)nbins * sizeof(unsigned long long), st));
+  k_stats_pdf<<<stats_blocks(G.n), STATS_THREADS, 0, st>>>(G, u, r, 1.0 / scale, lo, (double)nbins / (hi - lo), nbins, c);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(counts, c, (size_t)nbins * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return ACCLB_OK;
+}
+
+int accLB_stats_spectrum(const double* uhat, int nx, int ny, int nz, int ncomp, int nshell, double* E, void* scratch,
+                         size_t scratch_bytes, int device, void* stream) {
+  if (!stats_args(uhat, nx, ny, nz, scratch) || !E || ncomp < 1 || nshell < 1 || nshell > 4096)
+    return fail(ACCLB_EINVAL, "accLB_stats_spectrum: bad argument (1 <= nshell <= 4096)");
+  if (scratch_bytes < (size_t)nshell * sizeof(double) || ((size_t)scratch & 7)) return fail(ACCLB_EWORKSPACE, "accLB_stats_spectrum: scratch too small");
+  DeviceGuard guard_(device);
+  if (!guard_.ok) return fail(ACCLB_ECUDA, "accLB_stats_spectrum: cannot select device %d", device);
+  cudaStream_t st = (cudaStream_t)stream;
+  double* acc = (double*)scratch;
+  CK(cudaMemsetAsync(acc, 0, (size_t)nshell * sizeof(double), st));
+  const size_t nmode = (size_t)(nx / 2 + 1) * ny * nz;
+  k_stats_spectrum<<<stats_blocks(nmode), STATS_THREADS, (size_t)nshell * sizeof(double), st>>>(nx, ny, nz, ncomp, (const double2*)uhat, nshell, acc);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(E, acc, (size_t)nshell * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return ACCLB_OK;
+}
 
 }  // extern "C"
