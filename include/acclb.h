@@ -66,6 +66,10 @@ typedef struct {
   double rho_ref;    /* reference density of F^g; the mean density gives no net force on the periodic box (R31)   */
   int phi_integrator; /* 0: forward Euler, once per LB step (R13) | 1: three-stage SSP Runge-Kutta with u frozen at
                          time t, the normal recomputed from every stage field (R32)      */
+  /* moment-representation storage */
+  int moment_storage; /* 1: the state is the paper's ten macroscopic fields (p*, u, a) per node instead of 27 populations
+                         (160 B instead of 432 B moved per node and step; same results to rounding); single component,
+                         fp64 only (two_phase = 0, store_fp32 = 0) */
 } accLB_params;
 
 /* Bytes of device workspace accLB_create needs for this grid and these parameters; 0 on invalid arguments

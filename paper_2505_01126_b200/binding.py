@@ -37,6 +37,7 @@ class Params(C.Structure):
         ("store_fp32", C.c_int), ("host_staging", C.c_int),
         ("device", C.c_int), ("stream", C.c_void_p),
         ("gravity", C.c_double * 3), ("rho_ref", C.c_double), ("phi_integrator", C.c_int),
+        ("moment_storage", C.c_int),
     ]
 
 
@@ -91,10 +92,10 @@ def _check(code):
 
 def make_params(*, tau, two_phase=0, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0, width=4.0, force_type=0,
                 force_amp=0.0, force_k=1, store_fp32=0, host_staging=0, device=0, stream=None,
-                gravity=(0.0, 0.0, 0.0), rho_ref=0.0, phi_rk3=0):
+                gravity=(0.0, 0.0, 0.0), rho_ref=0.0, phi_rk3=0, moment_storage=0):
     return Params(tau, int(two_phase), rho_l, rho_g, sigma, mobility, width, int(force_type), force_amp, int(force_k),
                   int(store_fp32), int(host_staging), int(device), stream, (C.c_double * 3)(*gravity), rho_ref,
-                  int(phi_rk3))
+                  int(phi_rk3), int(moment_storage))
 
 
 def workspace_bytes(nx, ny, nz, params):

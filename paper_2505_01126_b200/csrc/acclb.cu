@@ -346,6 +346,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
 #include "twophase.cuh"
 #include "phase_rk.cuh"
 #include "stats.cuh"
+#include "momrep.cuh"
 
 // ================================================================================================== host / ABI
 using namespace acclb;
@@ -362,6 +363,7 @@ struct accLB_ctx {
   double* u;
   double* r;    // D lap phi - kappa div q of the current step (k_lb_tp -> k_advect)
   double* phis; // RK3 only: the second stage field
+  double* ms[2]; // moment_storage: the ten fields (p*, u, a) of every node, double-buffered (replaces f[])
   double* tabs;
   double* acc;
   CUtensorMap tmap[2];      // populations A / B as rank-3 tensors (x, y, z * 27 + i) for the TMA pull of k_lb_tp<FAST>,
@@ -462,6 +464,8 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
   if (p->force_type < 0 || p->force_type > 2) return false;
   if (!std::isfinite(p->gravity[0]) || !std::isfinite(p->gravity[1]) || !std::isfinite(p->gravity[2]) || !std::isfinite(p->rho_ref)) return false;
   if (p->phi_integrator < 0 || p->phi_integrator > 1) return false;
+  if (p->moment_storage < 0 || p->moment_storage > 1) return false;
+  if (p->moment_storage && (p->two_phase || p->store_fp32)) return false;  // single-phase fp64 only
   if (p->two_phase) {
     if (!(p->rho_l > 0.0) || !(p->rho_g > 0.0) || !(p->width > 0.0) || !(p->mobility >= 0.0)) return false;
   }
@@ -493,7 +497,7 @@ struct Carve {
 static Carve carve(int nx, int ny, int nz, const accLB_params* p) {
   const size_t n = (size_t)nx * ny * nz;
   Carve c;
-  c.f = align256(27 * n * (p->store_fp32 ? 4 : 8));
+  c.f = p->moment_storage ? align256(10 * n * 8) : align256(27 * n * (p->store_fp32 ? 4 : 8));
   c.phi = p->two_phase ? align256(n * 8) : 0;
   c.u = p->two_phase ? align256(3 * n * 8) : 0;
   c.r = p->two_phase ? align256(n * 8) : 0;
@@ -582,6 +586,23 @@ static int launch_advect(accLB_ctx* s, const double* phi_in, double* phi_out, co
   return ACCLB_OK;
 }
 
+// One single-phase step in the moment representation (k_mr_step, momrep.cuh).
+constexpr int MR_TX = 32, MR_TY = 8;
+static int launch_mr_step(accLB_ctx* s, int c, int d) {
+  using T = MomTile<MR_TX, MR_TY>;
+  auto kern = k_mr_step<MR_TX, MR_TY, 2>;
+  static thread_local int configured_device = -1;
+  if (configured_device != s->prm.device) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
+    configured_device = s->prm.device;
+  }
+  const int lz = s->lz;
+  const dim3 grid((s->nx + MR_TX - 1) / MR_TX, (s->ny + MR_TY - 1) / MR_TY, (s->nz + lz - 1) / lz);
+  LaunchScope ls(s, KIND_LB);
+  kern<<<grid, MR_TX * MR_TY, sizeof(T), s->stream>>>(s->kp, s->ms[c], s->ms[d], s->tabs, lz);
+  return ACCLB_OK;
+}
+
 // r = D lap phi - kappa div q of a Runge-Kutta stage field (k_geom_r, phase_rk.cuh).
 static int launch_geom_r(accLB_ctx* s, const double* phi_in) {
   using T = GeomTile<LBT_TX, LBT_TY>;
@@ -664,6 +685,7 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   char* w = (char*)workspace;
   s->f[0] = w; w += c.f;
   s->f[1] = w; w += c.f;
+  s->ms[0] = (double*)s->f[0]; s->ms[1] = (double*)s->f[1];
   s->phi[0] = p->two_phase ? (double*)w : nullptr; w += c.phi;
   s->phi[1] = p->two_phase ? (double*)w : nullptr; w += c.phi;
   s->u = p->two_phase ? (double*)w : nullptr; w += c.u;
@@ -735,6 +757,9 @@ int accLB_init(accLB_ctx* s, const double* rho, const double* u, const double* p
     CK(cudaMemcpyAsync(s->phi[0], phi, s->n * 8, cudaMemcpyDeviceToDevice, s->stream));
     int r = launch_lb_tp_any<MODE_INIT>(s, 0, 0, KIND_INIT, nullptr, nullptr, rho, u);
     if (r) return r;
+  } else if (s->prm.moment_storage) {
+    LaunchScope ls(s, KIND_INIT);
+    k_mr_init<<<blocks_for(s->n, 256), 256, 0, s->stream>>>(s->kp.G, rho, u, s->ms[0]);
   } else {
     LaunchScope ls(s, KIND_INIT);
     if (s->prm.store_fp32)
@@ -773,6 +798,9 @@ int accLB_step(accLB_ctx* s, int nsteps) {
       if (r) return r;
       r = launch_advect(s, s->phi[c], s->phi[d]);
       if (r) return r;
+    } else if (s->prm.moment_storage) {
+      int r = launch_mr_step(s, c, d);
+      if (r) return r;
     } else {
       LaunchScope ls(s, KIND_LB);
       if (s->prm.store_fp32)
@@ -798,6 +826,9 @@ int accLB_moments(accLB_ctx* s, double* rho, double* u, double* phi) {
       if (r) return r;
     }
     if (phi) CK(cudaMemcpyAsync(phi, s->phi[c], s->n * 8, cudaMemcpyDeviceToDevice, s->stream));
+  } else if (s->prm.moment_storage) {
+    LaunchScope ls(s, KIND_MOMENTS);
+    k_mr_moments<<<blocks_for(s->n, 256), 256, 0, s->stream>>>(s->kp.G, s->ms[c], rho, u);
   } else {
     LaunchScope ls(s, KIND_MOMENTS);
     if (s->prm.store_fp32)
@@ -820,6 +851,9 @@ int accLB_diagnostics(accLB_ctx* s, double* out, int n_out) {
   if (s->prm.two_phase) {
     int r = launch_lb_tp_any<MODE_DIAG>(s, c, c, KIND_DIAG, nullptr, s->acc);
     if (r) return r;
+  } else if (s->prm.moment_storage) {
+    LaunchScope ls(s, KIND_DIAG);
+    k_mr_diag<<<nb < 148u * 8u ? nb : 148u * 8u, 256, 0, s->stream>>>(s->kp, s->ms[c], s->tabs, s->acc);
   } else {
     LaunchScope ls(s, KIND_DIAG);
     if (s->prm.store_fp32)

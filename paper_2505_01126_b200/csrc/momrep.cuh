@@ -1,0 +1,278 @@
+// Moment-representation storage of the single-phase step, device side (sm_100a).  Part of the CUDA product path.
+//
+// the post-collision populations are "reconstructed directly from macroscopic fields, avoiding
+// direct access to full distribution functions", which "significantly reduces the memory footprint ... ten recovered
+// macroscopic fields".  Taken to its end the step is a closed map on those ten fields: the state is (p*, u, a) of every
+// node (10 doubles, double-buffered), and one step
+//   f_i(x, t+1) = f_i^eq(p*, u)(y) + (1 - omega) w_i H_i:a(y) / (2 cs4) + S_i(u, A)(y) / 2,  y = x - c_i     Eq. 6 (L85)
+//   p* = sum f_i,  m = sum f_i c_i,  Pi = sum f_i c_i c_i,  u = m + A/2,  a = Eq. 7 in closed form (O5')     L88, L92
+// moves 80 B read + 80 B written per node instead of 432 (A = F^b + F^g is recomputed from the force tables).  Exactly the
+// oracle's two-pass step, so the results are identical to rounding.
+//
+// k_mr_step: a block owns a TX x TY column of nodes and marches along z.  Iteration p: every thread rebuilds the 27
+// post-collision populations of its own node of SOURCE plane p (and of one node of the 1-wide rim: the neighbours of the
+// tile edge) from the ten fields (fetched one plane ahead by cp.async into the thread's own slots) and puts them into
+// shared memory; after a barrier it pulls its 27 incoming populations from the in-plane neighbours: the nine with
+// c_z = -1 complete the moments of consumer plane p-1 (node update, 10 aligned stores), the nine with c_z = 0 and +1 start
+// those of planes p and p+1 (carried in registers).
+#pragma once
+
+namespace acclb {
+
+constexpr int MR_FIELDS = 10;  // p*, u_x, u_y, u_z, a_xx, a_yy, a_zz, a_xy, a_xz, a_yz
+
+template <int TX, int TY>
+struct MomTile {
+  static constexpr int NX = TX + 2, NY = TY + 2;
+  double pop[Q][NY][NX];          // post-collision populations of the source plane, tile + rim 1
+  static constexpr int RIM = NX * NY - TX * TY;
+  double stage[MR_FIELDS][TX * TY];     // the ten fields of the next source plane at the thread's own node (own slots)
+  double stage_rim[MR_FIELDS][RIM];     // ... and at its rim item (threads tid < RIM)
+  double ftx[2][NX], fty[2][NY];  // sin / cos force-table entries of the tile's columns / rows incl. the rim (R20)
+};
+
+// state slab of plane z: [10][ny][nx]
+template <typename T>
+__device__ __forceinline__ T* mr_slab(T* s, const Grid& G, int z) {
+  T* p = s + (size_t)z * MR_FIELDS * ((size_t)G.nx * (size_t)G.ny);
+  asm("" : "+l"(p));
+  return p;
+}
+
+// moments of the nine populations with c_z = CZ (read through f_of(i), i = 9 (CZ + 1) .. 9 (CZ + 1) + 8), added to M
+template <int CZ, class F>
+__device__ __forceinline__ void mr_accumulate(F f_of, Moments& M) {
+#pragma unroll
+  for (int j = 0; j < 9; ++j) {
+    const int i = 9 * (CZ + 1) + j;
+    const int cx = cx_of(i), cy = cy_of(i);
+    const double f = f_of(i);
+    M.p += f;
+    if (cx == 1) M.m[0] += f;
+    if (cx == -1) M.m[0] -= f;
+    if (cy == 1) M.m[1] += f;
+    if (cy == -1) M.m[1] -= f;
+    if (CZ == 1) M.m[2] += f;
+    if (CZ == -1) M.m[2] -= f;
+    if (cx != 0) M.Pi[0] += f;
+    if (cy != 0) M.Pi[1] += f;
+    if (CZ != 0) M.Pi[2] += f;
+    if (cx * cy == 1) M.Pi[3] += f;
+    if (cx * cy == -1) M.Pi[3] -= f;
+    if (cx * CZ == 1) M.Pi[4] += f;
+    if (cx * CZ == -1) M.Pi[4] -= f;
+    if (cy * CZ == 1) M.Pi[5] += f;
+    if (cy * CZ == -1) M.Pi[5] -= f;
+  }
+}
+__device__ __forceinline__ void mr_zero(Moments& M) {
+  M.p = 0.0;
+  M.m[0] = M.m[1] = M.m[2] = 0.0;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) M.Pi[j] = 0.0;
+}
+
+template <int TX, int TY, int MINB>
+__global__ void __launch_bounds__(TX * TY, MINB)
+k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, const double* __restrict__ tabs, int lz) {
+  using T = MomTile<TX, TY>;
+  extern __shared__ __align__(128) unsigned char smem_lb[];
+  T& S = *reinterpret_cast<T*>(smem_lb);
+  constexpr int NT = TX * TY, NX = T::NX, NY = T::NY, RIM = NX * NY - NT;
+  static_assert(RIM <= NT, "at most one rim item per thread");
+  const Grid& G = P.G;
+  const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * lz;
+  const int z1 = min(z0 + lz, G.nz);
+  const int x = x0 + tx, y = y0 + ty;
+  const bool active = x < G.nx && y < G.ny;
+  const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
+  // the two source positions of this thread in the NY x NX plane: its own node, and a rim item (tid < RIM)
+  int rj = 0, ri = 0;
+  const bool has_rim = tid < RIM;
+  if (has_rim) {
+    if (tid < NX) { rj = 0; ri = tid; }
+    else if (tid < 2 * NX) { rj = NY - 1; ri = tid - NX; }
+    else { const int e = tid - 2 * NX; rj = 1 + (e >> 1); ri = (e & 1) ? NX - 1 : 0; }
+  }
+  const unsigned off_own = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
+  const unsigned off_rim = (unsigned)pmod(y0 - 1 + rj, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 1 + ri, G.nx);
+  // body-force table entries of the tile's columns and rows, rim included
+  if (P.force_type != 0) {
+    if (tid < NX) { const int xx = pmod(x0 - 1 + tid, G.nx); S.ftx[0][tid] = __ldg(tabs + xx); S.ftx[1][tid] = __ldg(tabs + G.nx + xx); }
+    if (tid >= 64 && tid < 64 + NY) {
+      const int yy = pmod(y0 - 1 + tid - 64, G.ny);
+      S.fty[0][tid - 64] = __ldg(tabs + 2 * G.nx + yy);
+      S.fty[1][tid - 64] = __ldg(tabs + 2 * G.nx + G.ny + yy);
+    }
+  }
+  auto fetch = [&](int p) {  // the ten fields of source plane p (any integer) into this thread's own slots
+    const double* sl = mr_slab(sin_, G, pmod(p, G.nz));
+#pragma unroll
+    for (int k = 0; k < MR_FIELDS; ++k) {
+      cp_async_f64(&S.stage[k][tid], sl + (unsigned)k * plane + off_own);
+      if (has_rim) cp_async_f64(&S.stage_rim[k][tid], sl + (unsigned)k * plane + off_rim);
+    }
+    cp_async_commit();
+  };
+  // acceleration A = F^b + F^g of a node of the plane (single component: rho == 1), R20 / R31
+  auto accel = [&](int j, int i, int zz, double (&A)[3]) {
+    A[0] = A[1] = A[2] = 0.0;
+    if (P.force_type != 0) {
+      const double fsz = __ldg(tabs + 2 * (G.nx + G.ny) + zz), fcz = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + zz);
+      const double fsx = S.ftx[0][i], fcx = S.ftx[1][i], fsy = S.fty[0][j], fcy = S.fty[1][j];
+      if (P.force_type == 1) { A[0] = P.force_amp * (fsz + fcy); A[1] = P.force_amp * (fsx + fcz); A[2] = P.force_amp * (fsy + fcx); }
+      else { A[0] = P.force_amp * fsy; A[1] = P.force_amp * fsz; A[2] = P.force_amp * fsx; }
+    }
+    if (P.buoyant) {
+      const double dr = 1.0 - P.rho_ref;
+      A[0] += dr * P.grav[0]; A[1] += dr * P.grav[1]; A[2] += dr * P.grav[2];
+    }
+  };
+  // Eq. 6 at a source node: the 27 post-collision populations from (p*, u, a) and A, into the shared plane
+  auto rebuild = [&](int slot, int j, int i, int zz) {
+    double c[MR_FIELDS];
+#pragma unroll
+    for (int k = 0; k < MR_FIELDS; ++k) c[k] = slot ? S.stage_rim[k][tid] : S.stage[k][tid];
+    double A[3];
+    accel(j, i, zz, A);
+    const double u[3] = {c[1], c[2], c[3]};
+    const double U[3] = {u[0] + 0.5 * A[0], u[1] + 0.5 * A[1], u[2] + 0.5 * A[2]};
+    double Tt[6];
+    Tt[0] = u[0] * u[0] + P.one_m_omega * c[4] + u[0] * A[0];
+    Tt[1] = u[1] * u[1] + P.one_m_omega * c[5] + u[1] * A[1];
+    Tt[2] = u[2] * u[2] + P.one_m_omega * c[6] + u[2] * A[2];
+    Tt[3] = u[0] * u[1] + P.one_m_omega * c[7] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
+    Tt[4] = u[0] * u[2] + P.one_m_omega * c[8] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
+    Tt[5] = u[1] * u[2] + P.one_m_omega * c[9] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
+    double f[Q];
+    hermite2_populations(c[0], U, Tt, f);
+#pragma unroll
+    for (int q = 0; q < Q; ++q) S.pop[q][j][i] = f[q];
+  };
+  __syncthreads();
+  fetch(z0 - 1);
+  Moments Mo, Mm;  // moments of consumer planes p-1 (two of three source planes in) and p (one in)
+  mr_zero(Mo);
+  mr_zero(Mm);
+  for (int p = z0 - 1; p <= z1; ++p) {
+    const int pw = pmod(p, G.nz);
+    cp_async_wait_all();
+    rebuild(0, ty + 1, tx + 1, pw);
+    if (has_rim) rebuild(1, rj, ri, pw);
+    if (p < z1) fetch(p + 1);  // own slots: free as soon as this thread has read them
+    __syncthreads();
+    auto pulled = [&](int i) { return S.pop[i][ty + 1 - cy_of(i)][tx + 1 - cx_of(i)]; };
+    // c_z = -1: source plane p feeds consumer plane p - 1 = its third and last contribution -> node update
+    mr_accumulate<-1>(pulled, Mo);
+    const int z = p - 1;
+    if (z >= z0 && z < z1 && active) {
+      double A[3];
+      accel(ty + 1, tx + 1, z, A);
+      const double u[3] = {Mo.m[0] + 0.5 * A[0], Mo.m[1] + 0.5 * A[1], Mo.m[2] + 0.5 * A[2]};  // a5 (R4)
+      double a[6];
+      hermite_coeff(Mo, u, A, a);                                                              // a6, Eq. 7 (O5')
+      double* o = mr_slab(sout, G, z) + off_own;
+      __stcs(o, Mo.p);
+      __stcs(o + plane, u[0]);
+      __stcs(o + 2u * plane, u[1]);
+      __stcs(o + 3u * plane, u[2]);
+#pragma unroll
+      for (int k = 0; k < 6; ++k) __stcs(o + (unsigned)(4 + k) * plane, a[k]);
+    }
+    Mo = Mm;
+    mr_accumulate<0>(pulled, Mo);   // consumer plane p: second contribution
+    mr_zero(Mm);
+    mr_accumulate<1>(pulled, Mm);   // consumer plane p + 1: first contribution
+    __syncthreads();                // the shared plane is rebuilt in the next iteration
+  }
+}
+
+// Initial state (R15): f = f^eq(p*, u0) - S/2 has p* = p*, u = m + A/2 = u0 and a = 0 (its non-equilibrium part is -S/2, which
+// Eq. 7 cancels), so the ten fields are (p*, u0, 0).
+__global__ void __launch_bounds__(256) k_mr_init(Grid G, const double* __restrict__ rho_in, const double* __restrict__ u_in,
+                                                 double* __restrict__ state) {
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= G.n) return;
+  const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
+  const unsigned z = k / plane, o = k - z * plane;
+  double* s = mr_slab(state, G, (int)z) + o;
+  s[0] = rho_in[k];
+  s[plane] = u_in[k];
+  s[2u * plane] = u_in[(size_t)G.n + k];
+  s[3u * plane] = u_in[2 * (size_t)G.n + k];
+#pragma unroll
+  for (int j = 4; j < MR_FIELDS; ++j) s[(unsigned)j * plane] = 0.0;
+}
+
+// a9: p*, u of the current state (a copy: they are stored)
+__global__ void __launch_bounds__(256) k_mr_moments(Grid G, const double* __restrict__ state, double* __restrict__ rho_out,
+                                                    double* __restrict__ u_out) {
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= G.n) return;
+  const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
+  const unsigned z = k / plane, o = k - z * plane;
+  const double* s = mr_slab(state, G, (int)z) + o;
+  if (rho_out) rho_out[k] = s[0];
+  if (u_out) {
+    u_out[k] = s[plane];
+    u_out[(size_t)G.n + k] = s[2u * plane];
+    u_out[2 * (size_t)G.n + k] = s[3u * plane];
+  }
+}
+
+// a9: diagnostics (R21) from the stored fields: KE, dissipation from a, sum p*, sum m (m = u - A/2), max |u|
+__global__ void __launch_bounds__(256) k_mr_diag(KP P, const double* __restrict__ state, const double* __restrict__ tabs,
+                                                 double* __restrict__ acc) {
+  const Grid& G = P.G;
+  const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
+  double s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (unsigned k = blockIdx.x * blockDim.x + threadIdx.x; k < G.n; k += gridDim.x * blockDim.x) {
+    const unsigned z = k / plane, o = k - z * plane;
+    const int y = (int)(o / (unsigned)G.nx), x = (int)(o - (unsigned)y * (unsigned)G.nx);
+    const double* c = mr_slab(state, G, (int)z) + o;
+    const double u[3] = {c[plane], c[2u * plane], c[3u * plane]};
+    double Fb[3];
+    body_force(P, tabs, x, y, (int)z, Fb);
+    if (P.buoyant) {
+      const double dr = 1.0 - P.rho_ref;
+      Fb[0] += dr * P.grav[0]; Fb[1] += dr * P.grav[1]; Fb[2] += dr * P.grav[2];
+    }
+    const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    double aa = 0.0;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      const double a = c[(unsigned)(4 + j) * plane];
+      aa += (j < 3 ? 1.0 : 2.0) * a * a;
+    }
+    s[0] += 0.5 * uu;
+    s[1] += P.eps_pref * aa;
+    s[3] += c[0];
+    s[4] += u[0] - 0.5 * Fb[0];
+    s[5] += u[1] - 0.5 * Fb[1];
+    s[6] += u[2] - 0.5 * Fb[2];
+    s[7] = fmax(s[7], sqrt(uu));
+  }
+  __shared__ double sh[8][8];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    double v = s[j];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double w = __shfl_xor_sync(0xffffffffu, v, o);
+      v = j < 7 ? v + w : fmax(v, w);
+    }
+    if (lane == 0) sh[j][wid] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 8) {
+    const int j = threadIdx.x;
+    double r = sh[j][0];
+    for (int w = 1; w < 8; ++w) r = j < 7 ? r + sh[j][w] : fmax(r, sh[j][w]);
+    if (j < 7) atomicAdd(acc + j, r);
+    else atomicMax(reinterpret_cast<unsigned long long*>(acc + 7), (unsigned long long)__double_as_longlong(r));
+  }
+}
+
+}  // namespace acclb
