@@ -34,8 +34,8 @@ UNIT = "GLUPS"
 # Algorithmic bytes per lattice update (DESIGN.md section 7 / SURVEY.md 8(d)):
 #   fused LB kernel: 27 populations read + 27 written, 8 B (fp64) or 4 B (fp32 storage) each;
 #   whole two-phase step: + phi read + phi written (8 B each).
-def lb_bytes_per_lup(fp32):
-    return 54 * (4 if fp32 else 8)
+def lb_bytes_per_lup(fp32, moment=False):
+    return 20 * 8 if moment else 54 * (4 if fp32 else 8)  # moment representation: 10 fields read + 10 written (8(f) #2)
 
 
 def step_bytes_per_lup(fp32, two_phase):
@@ -199,7 +199,7 @@ def dist_env():
 
 
 def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=True, variant=None, barrier=None,
-                 sample_clocks=True):
+                 sample_clocks=True, moment=False):
     """Time `steps` steps of the CUDA path on one GPU.  Returns a dict of raw measurements (this rank's)."""
     import numpy as np
     import torch
@@ -211,7 +211,7 @@ def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=T
     dev = torch.device("cuda", local_rank)
     stream = torch.cuda.current_stream(dev)
     sim = binding.AccLB(n, n, n, device=local_rank, stream=stream, store_fp32=int(fp32), host_staging=int(e2e),
-                        **cfg["params"])
+                        moment_storage=int(moment), **cfg["params"])
     if variant is not None:
         sim.set_variant(variant)
     h = {k: torch.from_numpy(np.ascontiguousarray(cfg[k])) for k in ("rho", "u", "phi") if cfg[k] is not None}
@@ -387,6 +387,16 @@ def run_cuda(args):
         # this process with the same steps / warm-up
         sp_cfg = make_workload("hit", args.n)
         sp = measure_cuda(sp_cfg, args.steps, args.warmup, local_rank=local_rank, fp32=bool(args.fp32), e2e=False)
+        mr = measure_cuda(sp_cfg, args.steps, args.warmup, local_rank=local_rank, e2e=False, moment=True) if not args.fp32 else None
+        if mr:  # the same step on the paper's ten macroscopic fields instead of 27 populations
+            g = n3 * args.steps / (mr["ms"] * 1e-3) / 1e9
+            line["single_phase_moment_storage"] = {
+                "workload": f"hit {args.n}^3 single-phase, state = (p*, u, a) per node (160 B/LUP moved, PAPER.md:L88, L118)",
+                "value": g, "unit": UNIT, "ms_per_step": mr["ms"] / args.steps, "gpu_launches": mr["launches"], "clocks": mr["clocks"],
+                "workspace_bytes": mr["workspace_bytes"],
+                "of_population_roofline": g * lb_bytes_per_lup(False) / hbm_peak()[0],
+                "of_own_roofline": g * lb_bytes_per_lup(False, True) / hbm_peak()[0],
+                "note": "SM-latency-bound (two barriers per plane, 16 warps per SM), not HBM-bound"}
         line["single_phase"] = {"workload": f"hit {args.n}^3 single-phase; " + WORKLOADS["hit"][1],
                                 "value": n3 * args.steps / (sp["ms"] * 1e-3) / 1e9, "unit": UNIT,
                                 "ms_per_step": sp["ms"] / args.steps, "gpu_launches": sp["launches"], "clocks": sp["clocks"],

@@ -145,10 +145,50 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
     Tt[3] = u[0] * u[1] + P.one_m_omega * c[7] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
     Tt[4] = u[0] * u[2] + P.one_m_omega * c[8] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
     Tt[5] = u[1] * u[2] + P.one_m_omega * c[9] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
-    double f[Q];
-    hermite2_populations(c[0], U, Tt, f);
+    if (slot == 0) {
+      double f[Q];
+      hermite2_populations(c[0], U, Tt, f);
 #pragma unroll
-    for (int q = 0; q < Q; ++q) S.pop[q][j][i] = f[q];
+      for (int q = 0; q < Q; ++q) S.pop[q][j][i] = f[q];
+    } else {
+      // a rim node only feeds the tile: the nine populations that point into it (c_y = +1 from the row below the tile,
+      // -1 from the row above, c_x = +1 / -1 from the columns left / right; a corner's are a subset of its row's)
+      const double e0 = c[0] - 1.5 * (Tt[0] + Tt[1] + Tt[2]);
+      auto one = [&](int q) {
+        const int cx = cx_of(q), cy = cy_of(q), cz = cz_of(q);
+        double cct = 0.0, cross = 0.0, cu = 0.0;
+        if (cx != 0) cct += Tt[0];
+        if (cy != 0) cct += Tt[1];
+        if (cz != 0) cct += Tt[2];
+        if (cx * cy == 1) cross += Tt[3];
+        if (cx * cy == -1) cross -= Tt[3];
+        if (cx * cz == 1) cross += Tt[4];
+        if (cx * cz == -1) cross -= Tt[4];
+        if (cy * cz == 1) cross += Tt[5];
+        if (cy * cz == -1) cross -= Tt[5];
+        cct += 2.0 * cross;
+        if (cx == 1) cu += U[0];
+        if (cx == -1) cu -= U[0];
+        if (cy == 1) cu += U[1];
+        if (cy == -1) cu -= U[1];
+        if (cz == 1) cu += U[2];
+        if (cz == -1) cu -= U[2];
+        S.pop[q][j][i] = w_of(q) * (e0 + 4.5 * cct) + (3.0 * w_of(q)) * cu;
+      };
+      if (j == 0) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) if (cy_of(q) == 1) one(q);
+      } else if (j == NY - 1) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) if (cy_of(q) == -1) one(q);
+      } else if (i == 0) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) if (cx_of(q) == 1) one(q);
+      } else {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) if (cx_of(q) == -1) one(q);
+      }
+    }
   };
   __syncthreads();
   fetch(z0 - 1);
