@@ -50,15 +50,7 @@ template <typename ST> struct Pop;
 template <> struct Pop<double> {
   static __device__ __forceinline__ double from_storage(double v, int) { return v; }
   static __device__ __forceinline__ double load(const double* p, int) { return __ldcs(p); }
-#if defined(XP_ST_CG)
-  static __device__ __forceinline__ void store(double* p, int, double v) { __stcg(p, v); }
-#elif defined(XP_ST_WT)
-  static __device__ __forceinline__ void store(double* p, int, double v) { __stwt(p, v); }
-#elif defined(XP_ST_DEF)
-  static __device__ __forceinline__ void store(double* p, int, double v) { *p = v; }
-#else
   static __device__ __forceinline__ void store(double* p, int, double v) { __stcs(p, v); }
-#endif
 };
 template <> struct Pop<float> {
   static __device__ __forceinline__ double from_storage(float v, int i) { return (double)v + w_of(i); }
@@ -473,10 +465,7 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
 }
 
 // Tile shapes of the two-phase kernels.
-#ifndef XP_MINB
-#define XP_MINB 2
-#endif
-constexpr int LBT_TX = 32, LBT_TY = 8, LBT_MINB = XP_MINB;
+constexpr int LBT_TX = 32, LBT_TY = 8, LBT_MINB = 2;
 constexpr int ADV_TX = 32, ADV_TY = 8;
 
 // Planes per block along z: enough blocks to load every SM a few times over, chunks of equal length, and no

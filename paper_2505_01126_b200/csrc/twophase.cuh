@@ -29,11 +29,7 @@
 
 namespace acclb {
 
-#ifdef XP_LZ
-constexpr int LZ_MAX = XP_LZ;
-#else
-constexpr int LZ_MAX = 64;  // planes per block along z, at most
-#endif
+constexpr int LZ_MAX = 64;  // planes per block along z, at most (128 and 256 were measured: no difference)
 
 __device__ __forceinline__ int pmod(int a, int n) {
   int r = a % n;
@@ -133,9 +129,6 @@ struct GeoTile {
   double e[FUSED ? 3 : 1][NA];  // own slots: phi + D lap phi (written when the plane is derived) - kappa div q (added at its
                                 // node update) of planes zc-2, zc-1, zc; slot = plane mod 3 (as col)
   double col[3][NA];      // own slots: phi of the three planes older than the ring (z-face window)
-#ifdef XP_PAD
-  double pad_[XP_PAD];
-#endif
   double acc[NA];         // own slot: phi(t+1) of the previous advected plane, still missing its upper z flux
 };
 
@@ -439,19 +432,13 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         }
       };
       derive(ty + 1, tx + 1, true);
-#ifndef XP_NORIM
       if (r1 >= 0) derive(r1 / T::NX, r1 % T::NX, false);
-#endif
     }
     // ---- FUSED a8: advective fluxes of plane p = zc - 2 through the faces inside the tile column (R12)
     //   x face (x, x+1): own u_x and the neighbour lane's;  y face (y, y+1): u_y of the row above (shared memory);
     //   z face (p-1, p): u_z carried along the march.  Faces on the tile's seams are left to k_seam.
     const int pz = zc - 2;
-#ifdef XP_NOADV
-    const bool adv = false;
-#else
     const bool adv = FUSED && (STEADY || pz >= z0);  // block-uniform; pz <= z1 - 1 because zc <= z1 + 1
-#endif
     double Tp = 0.0;                     // phi(t+1) of plane pz, accumulated
     if (FUSED) {
       const double* rq = ring(NR - 1);                   // plane zc-2 = pz, tile + halo 2
@@ -466,9 +453,6 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const bool xseam = tx == TX - 1 || x + 1 >= G.nx;  // the face to the right is a seam (or the thread idle)
         const bool yseam = ty == TY - 1 || y + 1 >= G.ny;
         const double* row = rq + (ty + 2) * PX + tx;       // phi(x-2 .. x+3) of the own row
-#ifdef XP_NOFLUX
-#define face_flux(a,b,c,d,e,f,g,h) ((a)+(b)+(c)+(d)+(e)+(f)+(g)+(h))
-#endif
         double Fx = face_flux(S.ux[tid], S.ux[xseam ? tid : tid + 1], row[0], row[1], row[2], row[3], row[4], row[5]);
         Fx = xseam ? 0.0 : Fx;
         double Fxl = __shfl_up_sync(0xffffffffu, Fx, 1);
@@ -484,9 +468,6 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         if (!STEADY) Fz = pz == z0 ? 0.0 : Fz;
         if (STEADY || (pz > z0 && active)) __stcs(phi_new + (size_t)(pz - 1) * plane + o2off, S.acc[tid] - Fz);  // plane pz-1 is complete
         Tp = S.e[cj][tid] - (Fx - Fxl) - Fy + Fz;
-#ifdef XP_NOFLUX
-#undef face_flux
-#endif
       }
       S.col[cj][tid] = php;  // plane zc-2 replaces plane zc-5
       cj = cj == 2 ? 0 : cj + 1;
