@@ -274,11 +274,12 @@ def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=T
 # kernel as it was at the commit named; when a kernel changes, its entry is re-measured or removed (then `traffic` is null).
 NCU_TRAFFIC = {
     ("k_lb_tp", "two", "fp64", 512): (61_964_335_000, "ncu --set full capture of k_lb_tp at commit d2abe4a, profiles/r02_ncu_full.txt"),
+    ("k_mr_step", "single", "fp64", 512): (22_305_399_000, "ncu --set full capture of k_mr_step, profiles/r02_ncu_full.txt (last block)"),
     ("k_lb", "single", "fp64", 512): (57_937_370_000, "ncu --set full capture of k_lb at commit d2abe4a, profiles/r02_ncu_full.txt"),
 }
 
 
-def roofline_of(meas, steps, fp32):
+def roofline_of(meas, steps, fp32, moment=False):
     """Roofline object.  `achieved`/`frac` are for the WHOLE step (the north-star's figure of merit): algorithmic bytes of a
     step (54 populations, + phi read + phi written when two-phase) x nodes / the CUDA-event time of the timed region.  The
     dominant kernel (largest summed CUDA-event time inside the timed region; events bracket every launch on the launching
@@ -288,8 +289,8 @@ def roofline_of(meas, steps, fp32):
     kernels = {k: v for k, v in meas["kernels"].items() if v[1]}
     name = max(kernels, key=lambda k: kernels[k][0])
     ms_k, cnt_k = kernels[name]
-    step_bpl = step_bytes_per_lup(fp32, meas["two_phase"])
-    bpl = step_bpl if name == "k_lb_tp" and "k_advect" not in kernels else lb_bytes_per_lup(fp32)
+    step_bpl = lb_bytes_per_lup(fp32, True) if moment else step_bytes_per_lup(fp32, meas["two_phase"])
+    bpl = step_bpl if moment or (name == "k_lb_tp" and "k_advect" not in kernels) else lb_bytes_per_lup(fp32)
     peak, how = hbm_peak()
     per_launch_ms = ms_k / max(cnt_k, 1)
     k_achieved = bpl * n3 / (per_launch_ms * 1e-3) / 1e9
@@ -347,7 +348,7 @@ def run_cuda(args):
     if args.rk3:
         cfg["params"]["phi_rk3"] = 1
     meas = measure_cuda(cfg, args.steps, args.warmup, local_rank=local_rank, world=world, fp32=bool(args.fp32),
-                        e2e=not args.no_e2e, variant=args.variant, barrier=barrier)
+                        e2e=not args.no_e2e, variant=args.variant, barrier=barrier, moment=bool(args.moment_storage))
     # replicas only: every rank ran the same-sized independent problem; time = max over ranks
     ms, e2e_ms = max_over_ranks([meas["ms"], meas.get("e2e", {}).get("ms", 0.0)], f"cuda:{local_rank}" if world > 1 else None)
     if rank != 0:
@@ -366,12 +367,13 @@ def run_cuda(args):
                                + WORKLOADS[args.workload][1],
                    "n": args.n, "two_phase": two_phase, "population_storage": "fp32" if args.fp32 else "fp64",
                    "phi_integrator": "ssp-rk3" if args.rk3 else "forward euler",
+                   "state": "ten macroscopic fields (p*, u, a) per node" if args.moment_storage else "27 populations per node",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"state of {meas['workspace_bytes'] / 1e9:.1f} GB streams through a 126 MB L2 every step; no flush needed",
                    "lups_per_step": world * n3},
         "clocks": meas["clocks"],
         "gpu_launches": meas["launches"],
-        "roofline": roofline_of(meas, args.steps, bool(args.fp32)),
+        "roofline": roofline_of(meas, args.steps, bool(args.fp32), moment=bool(args.moment_storage)),
         "diagnostics": {"before": meas["diag0"], "after": meas["diag1"]},
     }
     if "e2e" in meas:
@@ -451,6 +453,7 @@ def main():
     ap.add_argument("--fp32", type=int, default=0, help="1: fp32 population storage (arithmetic stays fp64)")
     ap.add_argument("--variant", type=int, default=None, help="kernel variant (accLB_set_variant), default = best")
     ap.add_argument("--rk3", type=int, default=0, help="1: SSP-RK3 integrator for phi (SURVEY 8(f) #1) instead of forward Euler")
+    ap.add_argument("--moment-storage", type=int, default=0, help="1: single-phase state = the ten fields (p*, u, a) per node (SURVEY 8(f) #2); use with --workload hit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-single", action="store_true", help="skip the single_phase leg of a two-phase run")

@@ -117,9 +117,10 @@ long long accLB_launch_count(const accLB_ctx* ctx);
  * LB step of single-phase contexts), 3 k_init, 4 k_moments, 5 k_diagnostics (single-phase kernels, or the tiled kernel
  * k_lb_tp in its init / moments / diagnostics mode for two-phase contexts), 6 k_lb_tp (the tiled two-phase step: LB +
  * geometry + advection), 7 k_seam (advective fluxes through the faces between its tile columns), 8 k_advect (variant 1
- * and the Runge-Kutta stages), 9 k_geom_r (D lap phi - kappa div q of a Runge-Kutta stage field); 0 and 2 are unused.
+ * and the Runge-Kutta stages), 9 k_geom_r (D lap phi - kappa div q of a Runge-Kutta stage field), 10 k_mr_step (the single-phase step on the ten
+ * macroscopic fields, moment_storage = 1); 0 and 2 are unused.
  * This is how bench.py measures kernel durations inside the timed region. */
-#define ACCLB_NKERNELS 10
+#define ACCLB_NKERNELS 11
 int accLB_profile(accLB_ctx* ctx, int enable);
 int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
 

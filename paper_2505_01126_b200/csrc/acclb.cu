@@ -433,7 +433,7 @@ struct LaunchScope {
   }
 };
 enum { KIND_LB = 1, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_LB_TP = 6,
-       KIND_SEAM = 7, KIND_ADVECT = 8, KIND_GEOM = 9 };
+       KIND_SEAM = 7, KIND_ADVECT = 8, KIND_GEOM = 9, KIND_MR = 10 };
 
 static thread_local char g_err[512] = "";
 
@@ -577,9 +577,10 @@ static int launch_advect(accLB_ctx* s, const double* phi_in, double* phi_out, co
 
 // One single-phase step in the moment representation (k_mr_step, momrep.cuh).
 constexpr int MR_TX = 32, MR_TY = 8;
-static int launch_mr_step(accLB_ctx* s, int c, int d) {
+template <bool FAST>
+static int launch_mr_step_t(accLB_ctx* s, int c, int d) {
   using T = MomTile<MR_TX, MR_TY>;
-  auto kern = k_mr_step<MR_TX, MR_TY, 2>;
+  auto kern = k_mr_step<MR_TX, MR_TY, 2, FAST>;
   static thread_local int configured_device = -1;
   if (configured_device != s->prm.device) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
@@ -587,9 +588,12 @@ static int launch_mr_step(accLB_ctx* s, int c, int d) {
   }
   const int lz = s->lz;
   const dim3 grid((s->nx + MR_TX - 1) / MR_TX, (s->ny + MR_TY - 1) / MR_TY, (s->nz + lz - 1) / lz);
-  LaunchScope ls(s, KIND_LB);
-  kern<<<grid, MR_TX * MR_TY, sizeof(T), s->stream>>>(s->kp, s->ms[c], s->ms[d], s->tabs, lz);
+  LaunchScope ls(s, KIND_MR);
+  kern<<<grid, MR_TX * MR_TY, sizeof(T), s->stream>>>(s->kp, s->ms[c], s->ms[d], s->tabs, lz, s->tmap[c]);
   return ACCLB_OK;
+}
+static int launch_mr_step(accLB_ctx* s, int c, int d) {
+  return s->tmap_ok ? launch_mr_step_t<true>(s, c, d) : launch_mr_step_t<false>(s, c, d);
 }
 
 // r = D lap phi - kappa div q of a Runge-Kutta stage field (k_geom_r, phase_rk.cuh).
@@ -625,7 +629,7 @@ static int make_tensor_maps(accLB_ctx* s) {
   if (s->prm.store_fp32) return 0;  // measured: with 128-byte rows the per-thread cp.async pull is faster (9.5 vs 9.9 ms)
   const size_t es = 8;
   if (s->nx % LBT_TX != 0 || s->ny % LBT_TY != 0) return 0;  // FAST: every tile full
-  const cuuint64_t dims[3] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny, (cuuint64_t)27 * s->nz};
+  const cuuint64_t dims[3] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny, (cuuint64_t)(s->prm.moment_storage ? 10 : 27) * s->nz};
   const cuuint64_t strides[2] = {(cuuint64_t)s->nx * es, (cuuint64_t)s->nx * s->ny * es};
   const cuuint32_t box[3] = {LBT_TX, LBT_TY, 1}, row[3] = {LBT_TX, 1, 1}, estr[3] = {1, 1, 1};
   for (int b = 0; b < 2; ++b) {
@@ -728,7 +732,7 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
     delete s;
     return fail(ACCLB_ECUDA, "accLB_create: table upload: %s", cudaGetErrorString(e));
   }
-  s->tmap_ok = p->two_phase ? make_tensor_maps(s) : 0;
+  s->tmap_ok = p->two_phase || p->moment_storage ? make_tensor_maps(s) : 0;
   *out = s;
   g_err[0] = 0;
   return ACCLB_OK;

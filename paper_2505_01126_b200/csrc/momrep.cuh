@@ -24,11 +24,14 @@ constexpr int MR_FIELDS = 10;  // p*, u_x, u_y, u_z, a_xx, a_yy, a_zz, a_xy, a_x
 template <int TX, int TY>
 struct MomTile {
   static constexpr int NX = TX + 2, NY = TY + 2;
-  double pop[Q][NY][NX];          // post-collision populations of the source plane, tile + rim 1
   static constexpr int RIM = NX * NY - TX * TY;
-  double stage[MR_FIELDS][TX * TY];     // the ten fields of the next source plane at the thread's own node (own slots)
-  double stage_rim[MR_FIELDS][RIM];     // ... and at its rim item (threads tid < RIM)
+  alignas(128) double stage[MR_FIELDS][TX * TY];  // the ten fields of the next source plane at the thread's own node: ten
+                                                  // TMA boxes (FAST), else one cp.async per thread and field (own slots)
+  double stage_rim[MR_FIELDS][RIM];     // ... and at its rim item (threads tid < RIM; cp.async: the rim wraps)
+  double pop[Q][NY][NX];                // post-collision populations of the source plane, tile + rim 1
+  unsigned long long sbar;              // mbarrier of the TMA staging
   double ftx[2][NX], fty[2][NY];  // sin / cos force-table entries of the tile's columns / rows incl. the rim (R20)
+  double ftz[2][LZ_MAX + 2];      // ... and of the chunk's planes z0-1 .. z1 (a global load per use would wait for L2)
 };
 
 // state slab of plane z: [10][ny][nx]
@@ -72,9 +75,12 @@ __device__ __forceinline__ void mr_zero(Moments& M) {
   for (int j = 0; j < 6; ++j) M.Pi[j] = 0.0;
 }
 
-template <int TX, int TY, int MINB>
+// FAST: the tile shape divides the box and the tensor map exists -- the own-node fields arrive by TMA (ten TX x TY boxes per
+// plane, one issuing thread), only the rim items by per-thread cp.async.
+template <int TX, int TY, int MINB, bool FAST>
 __global__ void __launch_bounds__(TX * TY, MINB)
-k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, const double* __restrict__ tabs, int lz) {
+k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, const double* __restrict__ tabs, int lz,
+          const __grid_constant__ CUtensorMap tmap_in) {
   using T = MomTile<TX, TY>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
@@ -90,10 +96,13 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
   // the two source positions of this thread in the NY x NX plane: its own node, and a rim item (tid < RIM)
   int rj = 0, ri = 0;
   const bool has_rim = tid < RIM;
+  // warp 0: the row below the tile (j = 0, i = 1..TX), warp 1: the row above (j = NY-1), then the two columns with the
+  // corners (2 NY items): every warp that has rim items runs ONE code path for them
+  static_assert(TX == 32 && 2 * TX + 2 * NY == RIM, "rim items: two full warps for the rows, 2 NY lanes for the columns");
   if (has_rim) {
-    if (tid < NX) { rj = 0; ri = tid; }
-    else if (tid < 2 * NX) { rj = NY - 1; ri = tid - NX; }
-    else { const int e = tid - 2 * NX; rj = 1 + (e >> 1); ri = (e & 1) ? NX - 1 : 0; }
+    if (tid < TX) { rj = 0; ri = tid + 1; }
+    else if (tid < 2 * TX) { rj = NY - 1; ri = tid - TX + 1; }
+    else { const int e = tid - 2 * TX; rj = e >> 1; ri = (e & 1) ? NX - 1 : 0; }
   }
   const unsigned off_own = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
   const unsigned off_rim = (unsigned)pmod(y0 - 1 + rj, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 1 + ri, G.nx);
@@ -105,21 +114,39 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
       S.fty[0][tid - 64] = __ldg(tabs + 2 * G.nx + yy);
       S.fty[1][tid - 64] = __ldg(tabs + 2 * G.nx + G.ny + yy);
     }
+    if (tid >= 128 && tid < 128 + (z1 - z0) + 2) {
+      const int zz = pmod(z0 - 1 + tid - 128, G.nz);
+      S.ftz[0][tid - 128] = __ldg(tabs + 2 * (G.nx + G.ny) + zz);
+      S.ftz[1][tid - 128] = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + zz);
+    }
   }
   auto fetch = [&](int p) {  // the ten fields of source plane p (any integer) into this thread's own slots
     const double* sl = mr_slab(sin_, G, pmod(p, G.nz));
 #pragma unroll
     for (int k = 0; k < MR_FIELDS; ++k) {
-      cp_async_f64(&S.stage[k][tid], sl + (unsigned)k * plane + off_own);
+      if (!FAST) cp_async_f64(&S.stage[k][tid], sl + (unsigned)k * plane + off_own);
       if (has_rim) cp_async_f64(&S.stage_rim[k][tid], sl + (unsigned)k * plane + off_rim);
     }
     cp_async_commit();
   };
+  auto tma_fetch = [&](int p) {  // FAST: the ten own-node boxes of source plane p, by one thread, after a block barrier
+    if (tid == NT / 2) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_arrive_expect_tx(&S.sbar, (unsigned)(MR_FIELDS * NT * sizeof(double)));
+      const int slab0 = pmod(p, G.nz) * MR_FIELDS;
+#pragma unroll
+      for (int k = 0; k < MR_FIELDS; ++k) tma_load_box(&S.stage[k][0], &tmap_in, x0, y0, slab0 + k, &S.sbar);
+    }
+  };
+  if (FAST && tid == 0) {
+    mbar_init(&S.sbar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   // acceleration A = F^b + F^g of a node of the plane (single component: rho == 1), R20 / R31
-  auto accel = [&](int j, int i, int zz, double (&A)[3]) {
+  auto accel = [&](int j, int i, int zl, double (&A)[3]) {  // zl = plane - (z0 - 1)
     A[0] = A[1] = A[2] = 0.0;
     if (P.force_type != 0) {
-      const double fsz = __ldg(tabs + 2 * (G.nx + G.ny) + zz), fcz = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + zz);
+      const double fsz = S.ftz[0][zl], fcz = S.ftz[1][zl];
       const double fsx = S.ftx[0][i], fcx = S.ftx[1][i], fsy = S.fty[0][j], fcy = S.fty[1][j];
       if (P.force_type == 1) { A[0] = P.force_amp * (fsz + fcy); A[1] = P.force_amp * (fsx + fcz); A[2] = P.force_amp * (fsy + fcx); }
       else { A[0] = P.force_amp * fsy; A[1] = P.force_amp * fsz; A[2] = P.force_amp * fsx; }
@@ -130,12 +157,12 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
     }
   };
   // Eq. 6 at a source node: the 27 post-collision populations from (p*, u, a) and A, into the shared plane
-  auto rebuild = [&](int slot, int j, int i, int zz) {
+  auto rebuild = [&](int slot, int j, int i, int zl) {
     double c[MR_FIELDS];
 #pragma unroll
     for (int k = 0; k < MR_FIELDS; ++k) c[k] = slot ? S.stage_rim[k][tid] : S.stage[k][tid];
     double A[3];
-    accel(j, i, zz, A);
+    accel(j, i, zl, A);
     const double u[3] = {c[1], c[2], c[3]};
     const double U[3] = {u[0] + 0.5 * A[0], u[1] + 0.5 * A[1], u[2] + 0.5 * A[2]};
     double Tt[6];
@@ -151,64 +178,59 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
 #pragma unroll
       for (int q = 0; q < Q; ++q) S.pop[q][j][i] = f[q];
     } else {
-      // a rim node only feeds the tile: the nine populations that point into it (c_y = +1 from the row below the tile,
-      // -1 from the row above, c_x = +1 / -1 from the columns left / right; a corner's are a subset of its row's)
+      // a rim node only feeds the tile: the nine populations that point into it -- c_y = s (s = +1 from the row below the
+      // tile, -1 from the row above) or c_x = s (columns left / right; a corner's three are among its column's nine).
+      // One instruction sequence per kind, the side entering as the sign s.
       const double e0 = c[0] - 1.5 * (Tt[0] + Tt[1] + Tt[2]);
-      auto one = [&](int q) {
-        const int cx = cx_of(q), cy = cy_of(q), cz = cz_of(q);
-        double cct = 0.0, cross = 0.0, cu = 0.0;
-        if (cx != 0) cct += Tt[0];
-        if (cy != 0) cct += Tt[1];
-        if (cz != 0) cct += Tt[2];
-        if (cx * cy == 1) cross += Tt[3];
-        if (cx * cy == -1) cross -= Tt[3];
-        if (cx * cz == 1) cross += Tt[4];
-        if (cx * cz == -1) cross -= Tt[4];
-        if (cy * cz == 1) cross += Tt[5];
-        if (cy * cz == -1) cross -= Tt[5];
-        cct += 2.0 * cross;
-        if (cx == 1) cu += U[0];
-        if (cx == -1) cu -= U[0];
-        if (cy == 1) cu += U[1];
-        if (cy == -1) cu -= U[1];
-        if (cz == 1) cu += U[2];
-        if (cz == -1) cu -= U[2];
-        S.pop[q][j][i] = w_of(q) * (e0 + 4.5 * cct) + (3.0 * w_of(q)) * cu;
-      };
-      if (j == 0) {
+      const bool row = tid < 2 * TX;
+      const double sgn = row ? (j == 0 ? 1.0 : -1.0) : (i == 0 ? 1.0 : -1.0);
+      // fixed direction f (y for a row item, x for a column item), free in-plane direction g, and z
+      const double Tf = row ? Tt[1] : Tt[0], Tg = row ? Tt[0] : Tt[1];
+      const double Tfg = sgn * Tt[3], Tfz = sgn * (row ? Tt[5] : Tt[4]), Tgz = row ? Tt[4] : Tt[5];
+      const double Uf = sgn * (row ? U[1] : U[0]), Ug = row ? U[0] : U[1];
+      const int qf = (sgn > 0.0 ? 2 : 0) * (row ? 3 : 1), qg = row ? 1 : 3;  // population index = qf + (cg + 1) qg + 9 (cz + 1)
+      double* dst = &S.pop[0][j][i] + (size_t)qf * (NY * NX);
 #pragma unroll
-        for (int q = 0; q < Q; ++q) if (cy_of(q) == 1) one(q);
-      } else if (j == NY - 1) {
+      for (int cz = -1; cz <= 1; ++cz)
 #pragma unroll
-        for (int q = 0; q < Q; ++q) if (cy_of(q) == -1) one(q);
-      } else if (i == 0) {
-#pragma unroll
-        for (int q = 0; q < Q; ++q) if (cx_of(q) == 1) one(q);
-      } else {
-#pragma unroll
-        for (int q = 0; q < Q; ++q) if (cx_of(q) == -1) one(q);
-      }
+        for (int cg = -1; cg <= 1; ++cg) {
+          const int nnz = 1 + (cg != 0) + (cz != 0);
+          const double w = nnz == 1 ? 2.0 / 27.0 : nnz == 2 ? 1.0 / 54.0 : 1.0 / 216.0;
+          double cct = Tf, cross = 0.0, cu = Uf;
+          if (cg != 0) cct += Tg;
+          if (cz != 0) cct += Tt[2];
+          if (cg == 1) { cross += Tfg; cu += Ug; }
+          if (cg == -1) { cross -= Tfg; cu -= Ug; }
+          if (cz == 1) { cross += Tfz; cu += U[2]; }
+          if (cz == -1) { cross -= Tfz; cu -= U[2]; }
+          if (cg * cz == 1) cross += Tgz;
+          if (cg * cz == -1) cross -= Tgz;
+          cct += 2.0 * cross;
+          dst[(size_t)((cg + 1) * qg + 9 * (cz + 1)) * (NY * NX)] = w * (e0 + 4.5 * cct) + (3.0 * w) * cu;
+        }
     }
   };
   __syncthreads();
   fetch(z0 - 1);
+  if (FAST) tma_fetch(z0 - 1);
   Moments Mo, Mm;  // moments of consumer planes p-1 (two of three source planes in) and p (one in)
   mr_zero(Mo);
   mr_zero(Mm);
   for (int p = z0 - 1; p <= z1; ++p) {
-    const int pw = pmod(p, G.nz);
     cp_async_wait_all();
-    rebuild(0, ty + 1, tx + 1, pw);
-    if (has_rim) rebuild(1, rj, ri, pw);
+    if (FAST) mbar_wait(&S.sbar, (unsigned)(p - (z0 - 1)) & 1u);
+    rebuild(0, ty + 1, tx + 1, p - (z0 - 1));
+    if (has_rim) rebuild(1, rj, ri, p - (z0 - 1));
     if (p < z1) fetch(p + 1);  // own slots: free as soon as this thread has read them
     __syncthreads();
+    if (FAST && p < z1) tma_fetch(p + 1);  // every thread has read its fields of plane p (barrier above)
     auto pulled = [&](int i) { return S.pop[i][ty + 1 - cy_of(i)][tx + 1 - cx_of(i)]; };
     // c_z = -1: source plane p feeds consumer plane p - 1 = its third and last contribution -> node update
     mr_accumulate<-1>(pulled, Mo);
     const int z = p - 1;
     if (z >= z0 && z < z1 && active) {
       double A[3];
-      accel(ty + 1, tx + 1, z, A);
+      accel(ty + 1, tx + 1, z - (z0 - 1), A);
       const double u[3] = {Mo.m[0] + 0.5 * A[0], Mo.m[1] + 0.5 * A[1], Mo.m[2] + 0.5 * A[2]};  // a5 (R4)
       double a[6];
       hermite_coeff(Mo, u, A, a);                                                              // a6, Eq. 7 (O5')
