@@ -149,7 +149,14 @@ class AccLB:
             (t.device, t.dtype, tuple(t.shape), shape)
         return t.data_ptr()
 
+    def _on_stream(self):
+        """The context enqueues on the stream it was created with; the caller's tensors must be ordered on the same one."""
+        cur = self._torch.cuda.current_stream(self.device)
+        assert cur.cuda_stream == self.stream.cuda_stream, \
+            "AccLB was created on another stream: call it under `with torch.cuda.stream(sim.stream)` (or synchronise)"
+
     def init(self, rho, u, phi=None):
+        self._on_stream()
         _check(load().accLB_init(self._h, self._dev(rho, self.shape), self._dev(u, (3,) + self.shape),
                                  self._dev(phi, self.shape) if phi is not None else None))
 
@@ -157,6 +164,7 @@ class AccLB:
         _check(load().accLB_step(self._h, int(nsteps)))
 
     def moments(self, rho=None, u=None, phi=None):
+        self._on_stream()
         torch = self._torch
         kw = dict(dtype=torch.float64, device=self.device)
         rho = torch.empty(self.shape, **kw) if rho is None else rho
@@ -174,6 +182,7 @@ class AccLB:
 
     def run_host(self, rho, u, phi, nsteps, rho_out=None, u_out=None, phi_out=None, diag=True):
         """Host-buffer path: CPU tensors (pinned for asynchronous copies) in and out."""
+        self._on_stream()
         def hp(t, shape):
             if t is None:
                 return None

@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(128) k_init(KP P, const double* __restrict__ r
   double A[3], rho;
   node_accel(P, tabs, x, y, z, A, rho);
   const double p = rho_in[k];
-  const double u[3] = {u_in[k], u_in[P.G.n + k], u_in[2u * P.G.n + k]};
+  const double u[3] = {u_in[k], u_in[(size_t)P.G.n + k], u_in[2 * (size_t)P.G.n + k]};  // (3 n may exceed 2^32)
   const double U[3] = {u[0] - 0.5 * A[0], u[1] - 0.5 * A[1], u[2] - 0.5 * A[2]};
   double T[6];
   T[0] = u[0] * u[0] - u[0] * A[0];
@@ -261,8 +261,8 @@ __global__ void __launch_bounds__(128) k_moments(KP P, const ST* __restrict__ fi
   if (rho_out) rho_out[k] = M.p;
   if (u_out) {
     u_out[k] = M.m[0] + 0.5 * A[0];
-    u_out[P.G.n + k] = M.m[1] + 0.5 * A[1];
-    u_out[2u * P.G.n + k] = M.m[2] + 0.5 * A[2];
+    u_out[(size_t)P.G.n + k] = M.m[1] + 0.5 * A[1];
+    u_out[2 * (size_t)P.G.n + k] = M.m[2] + 0.5 * A[2];
   }
 }
 
