@@ -77,21 +77,23 @@ __device__ __forceinline__ void mr_zero(Moments& M) {
 
 // FAST: the tile shape divides the box and the tensor map exists -- the own-node fields arrive by TMA (ten TX x TY boxes per
 // plane, one issuing thread), only the rim items by per-thread cp.async.
-template <int TX, int TY, int MINB, bool FAST>
-__global__ void __launch_bounds__(TX * TY, MINB)
+// NPT: nodes per thread (rows ty + r TY / NPT of the tile).  Two nodes per thread (two independent chains per thread, half
+// the warps per block barrier) were measured and are no faster than one (7.27 vs 7.18 ms at 512^3): the limit is the
+// shared-memory traffic of the rebuilt populations, not the issue rate per warp.
+template <int TX, int TY, int NPT, int MINB, bool FAST>
+__global__ void __launch_bounds__(TX * TY / NPT, MINB)
 k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, const double* __restrict__ tabs, int lz,
           const __grid_constant__ CUtensorMap tmap_in) {
   using T = MomTile<TX, TY>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
-  constexpr int NT = TX * TY, NX = T::NX, NY = T::NY, RIM = NX * NY - NT;
-  static_assert(RIM <= NT, "at most one rim item per thread");
+  constexpr int NT = TX * TY / NPT, NX = T::NX, NY = T::NY, RIM = NX * NY - TX * TY, RY = TY / NPT;
+  static_assert(RIM <= NT && TY % NPT == 0, "at most one rim item per thread");
   const Grid& G = P.G;
   const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * lz;
   const int z1 = min(z0 + lz, G.nz);
-  const int x = x0 + tx, y = y0 + ty;
-  const bool active = x < G.nx && y < G.ny;
+  const int x = x0 + tx;
   const unsigned plane = (unsigned)G.nx * (unsigned)G.ny;
   // the two source positions of this thread in the NY x NX plane: its own node, and a rim item (tid < RIM)
   int rj = 0, ri = 0;
@@ -104,7 +106,14 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
     else if (tid < 2 * TX) { rj = NY - 1; ri = tid - TX + 1; }
     else { const int e = tid - 2 * TX; rj = e >> 1; ri = (e & 1) ? NX - 1 : 0; }
   }
-  const unsigned off_own = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
+  unsigned off_own[NPT];
+  bool active[NPT];
+#pragma unroll
+  for (int r = 0; r < NPT; ++r) {
+    const int y = y0 + ty + r * RY;
+    off_own[r] = (unsigned)pmod(y, G.ny) * (unsigned)G.nx + (unsigned)pmod(x, G.nx);
+    active[r] = x < G.nx && y < G.ny;
+  }
   const unsigned off_rim = (unsigned)pmod(y0 - 1 + rj, G.ny) * (unsigned)G.nx + (unsigned)pmod(x0 - 1 + ri, G.nx);
   // body-force table entries of the tile's columns and rows, rim included
   if (P.force_type != 0) {
@@ -114,17 +123,20 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
       S.fty[0][tid - 64] = __ldg(tabs + 2 * G.nx + yy);
       S.fty[1][tid - 64] = __ldg(tabs + 2 * G.nx + G.ny + yy);
     }
-    if (tid >= 128 && tid < 128 + (z1 - z0) + 2) {
-      const int zz = pmod(z0 - 1 + tid - 128, G.nz);
-      S.ftz[0][tid - 128] = __ldg(tabs + 2 * (G.nx + G.ny) + zz);
-      S.ftz[1][tid - 128] = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + zz);
+    for (int t = tid; t < (z1 - z0) + 2; t += NT) {
+      const int zz = pmod(z0 - 1 + t, G.nz);
+      S.ftz[0][t] = __ldg(tabs + 2 * (G.nx + G.ny) + zz);
+      S.ftz[1][t] = __ldg(tabs + 2 * (G.nx + G.ny) + G.nz + zz);
     }
   }
   auto fetch = [&](int p) {  // the ten fields of source plane p (any integer) into this thread's own slots
     const double* sl = mr_slab(sin_, G, pmod(p, G.nz));
 #pragma unroll
     for (int k = 0; k < MR_FIELDS; ++k) {
-      if (!FAST) cp_async_f64(&S.stage[k][tid], sl + (unsigned)k * plane + off_own);
+      if (!FAST) {
+#pragma unroll
+        for (int r = 0; r < NPT; ++r) cp_async_f64(&S.stage[k][r * NT + tid], sl + (unsigned)k * plane + off_own[r]);
+      }
       if (has_rim) cp_async_f64(&S.stage_rim[k][tid], sl + (unsigned)k * plane + off_rim);
     }
     cp_async_commit();
@@ -132,7 +144,7 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
   auto tma_fetch = [&](int p) {  // FAST: the ten own-node boxes of source plane p, by one thread, after a block barrier
     if (tid == NT / 2) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_arrive_expect_tx(&S.sbar, (unsigned)(MR_FIELDS * NT * sizeof(double)));
+      mbar_arrive_expect_tx(&S.sbar, (unsigned)(MR_FIELDS * TX * TY * sizeof(double)));
       const int slab0 = pmod(p, G.nz) * MR_FIELDS;
 #pragma unroll
       for (int k = 0; k < MR_FIELDS; ++k) tma_load_box(&S.stage[k][0], &tmap_in, x0, y0, slab0 + k, &S.sbar);
@@ -157,10 +169,10 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
     }
   };
   // Eq. 6 at a source node: the 27 post-collision populations from (p*, u, a) and A, into the shared plane
-  auto rebuild = [&](int slot, int j, int i, int zl) {
+  auto rebuild = [&](int slot, int j, int i, int zl) {  // slot = r (own node of row r) or -1 (rim item)
     double c[MR_FIELDS];
 #pragma unroll
-    for (int k = 0; k < MR_FIELDS; ++k) c[k] = slot ? S.stage_rim[k][tid] : S.stage[k][tid];
+    for (int k = 0; k < MR_FIELDS; ++k) c[k] = slot < 0 ? S.stage_rim[k][tid] : S.stage[k][slot * NT + tid];
     double A[3];
     accel(j, i, zl, A);
     const double u[3] = {c[1], c[2], c[3]};
@@ -172,7 +184,7 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
     Tt[3] = u[0] * u[1] + P.one_m_omega * c[7] + 0.5 * (u[0] * A[1] + u[1] * A[0]);
     Tt[4] = u[0] * u[2] + P.one_m_omega * c[8] + 0.5 * (u[0] * A[2] + u[2] * A[0]);
     Tt[5] = u[1] * u[2] + P.one_m_omega * c[9] + 0.5 * (u[1] * A[2] + u[2] * A[1]);
-    if (slot == 0) {
+    if (slot >= 0) {
       double f[Q];
       hermite2_populations(c[0], U, Tt, f);
 #pragma unroll
@@ -213,39 +225,44 @@ k_mr_step(KP P, const double* __restrict__ sin_, double* __restrict__ sout, cons
   __syncthreads();
   fetch(z0 - 1);
   if (FAST) tma_fetch(z0 - 1);
-  Moments Mo, Mm;  // moments of consumer planes p-1 (two of three source planes in) and p (one in)
-  mr_zero(Mo);
-  mr_zero(Mm);
+  Moments Mo[NPT], Mm[NPT];  // moments of consumer planes p-1 (two of three source planes in) and p (one in)
+#pragma unroll
+  for (int r = 0; r < NPT; ++r) { mr_zero(Mo[r]); mr_zero(Mm[r]); }
   for (int p = z0 - 1; p <= z1; ++p) {
     cp_async_wait_all();
     if (FAST) mbar_wait(&S.sbar, (unsigned)(p - (z0 - 1)) & 1u);
-    rebuild(0, ty + 1, tx + 1, p - (z0 - 1));
-    if (has_rim) rebuild(1, rj, ri, p - (z0 - 1));
+#pragma unroll
+    for (int r = 0; r < NPT; ++r) rebuild(r, ty + r * RY + 1, tx + 1, p - (z0 - 1));
+    if (has_rim) rebuild(-1, rj, ri, p - (z0 - 1));
     if (p < z1) fetch(p + 1);  // own slots: free as soon as this thread has read them
     __syncthreads();
     if (FAST && p < z1) tma_fetch(p + 1);  // every thread has read its fields of plane p (barrier above)
-    auto pulled = [&](int i) { return S.pop[i][ty + 1 - cy_of(i)][tx + 1 - cx_of(i)]; };
-    // c_z = -1: source plane p feeds consumer plane p - 1 = its third and last contribution -> node update
-    mr_accumulate<-1>(pulled, Mo);
     const int z = p - 1;
-    if (z >= z0 && z < z1 && active) {
-      double A[3];
-      accel(ty + 1, tx + 1, z - (z0 - 1), A);
-      const double u[3] = {Mo.m[0] + 0.5 * A[0], Mo.m[1] + 0.5 * A[1], Mo.m[2] + 0.5 * A[2]};  // a5 (R4)
-      double a[6];
-      hermite_coeff(Mo, u, A, a);                                                              // a6, Eq. 7 (O5')
-      double* o = mr_slab(sout, G, z) + off_own;
-      __stcs(o, Mo.p);
-      __stcs(o + plane, u[0]);
-      __stcs(o + 2u * plane, u[1]);
-      __stcs(o + 3u * plane, u[2]);
 #pragma unroll
-      for (int k = 0; k < 6; ++k) __stcs(o + (unsigned)(4 + k) * plane, a[k]);
+    for (int r = 0; r < NPT; ++r) {
+      const int jy = ty + r * RY + 1;
+      auto pulled = [&](int i) { return S.pop[i][jy - cy_of(i)][tx + 1 - cx_of(i)]; };
+      // c_z = -1: source plane p feeds consumer plane p - 1 = its third and last contribution -> node update
+      mr_accumulate<-1>(pulled, Mo[r]);
+      if (z >= z0 && z < z1 && active[r]) {
+        double A[3];
+        accel(jy, tx + 1, z - (z0 - 1), A);
+        const double u[3] = {Mo[r].m[0] + 0.5 * A[0], Mo[r].m[1] + 0.5 * A[1], Mo[r].m[2] + 0.5 * A[2]};  // a5 (R4)
+        double a[6];
+        hermite_coeff(Mo[r], u, A, a);                                                                    // a6, Eq. 7 (O5')
+        double* o = mr_slab(sout, G, z) + off_own[r];
+        __stcs(o, Mo[r].p);
+        __stcs(o + plane, u[0]);
+        __stcs(o + 2u * plane, u[1]);
+        __stcs(o + 3u * plane, u[2]);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) __stcs(o + (unsigned)(4 + k) * plane, a[k]);
+      }
+      Mo[r] = Mm[r];
+      mr_accumulate<0>(pulled, Mo[r]);   // consumer plane p: second contribution
+      mr_zero(Mm[r]);
+      mr_accumulate<1>(pulled, Mm[r]);   // consumer plane p + 1: first contribution
     }
-    Mo = Mm;
-    mr_accumulate<0>(pulled, Mo);   // consumer plane p: second contribution
-    mr_zero(Mm);
-    mr_accumulate<1>(pulled, Mm);   // consumer plane p + 1: first contribution
     __syncthreads();                // the shared plane is rebuilt in the next iteration
   }
 }
