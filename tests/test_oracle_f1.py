@@ -195,3 +195,22 @@ def test_rk3_removes_the_forward_euler_amplification():
         if rk3:
             assert np.abs(phi - phi0).max() < 2e-3                   # back where it started after one period
     assert abs(amp[1] - 1.0) < 1e-3 and amp[0] - 1.0 > 0.03, amp
+
+
+# ------------------------------------------------------------------ the stored Laplace study (oracle only)
+def test_stored_laplace_study_matches_the_lattice_normalisation():
+    """tests/golden/laplace_oracle.txt is written by oracle/laplace_study.py (oracle only, to equilibrium: 1.5 R^2 / nu steps).
+    The pressure jump converges, with R, to the lattice value of the normalisation integral of reading R8:
+    (3 delta / 2) sum_x (D phi)^2 = 0.9391 for the tanh profile at delta = 4 with the central difference of PAPER.md:L104
+    (a closed form, evaluated here), not to 1: within 3 % of it at R = 12 and 16, both measurement methods agreeing."""
+    from pathlib import Path
+
+    x = np.arange(-200, 201, dtype=np.float64)
+    phi = 0.5 * (1.0 + np.tanh(2.0 * x / 4.0))
+    lat = 1.5 * 4.0 * float(((0.5 * (phi[2:] - phi[:-2])) ** 2).sum())
+    assert abs(lat - 0.9391) < 1e-4
+    rows = [l.split() for l in (Path(__file__).parent / "golden" / "laplace_oracle.txt").read_text().splitlines() if l and l[0] != "#"]
+    assert {(float(r[0]), float(r[2])) for r in rows} >= {(12.0, 1.0), (12.0, 10.0), (16.0, 1.0), (16.0, 10.0)}
+    for r in rows:
+        A, B = float(r[4]), float(r[5])
+        assert abs(A - B) < 0.005 and abs(B / lat - 1.0) < 0.035, r
