@@ -1,28 +1,30 @@
 // Two-phase hot path on shared-memory tiles, device side (sm_100a).  Part of the CUDA product path.
 //
-// One two-phase step is the fused kernel k_lb_tp<FUSED = true> plus the small seam kernel k_seam:
+// One two-phase step is the tiled kernel k_lb_tp<MODE_FUSED> plus the small seam kernel k_seam:
 //   k_lb_tp     rows a1-a8.  A block owns a TX x TY column of nodes and marches along z.
 //               Per plane it stages phi (halo 2) in shared memory, derives the interface normal n, the sharpening flux
 //               q = phi (1 - phi) n and |grad phi| ONCE per node of the tile + 1 rim (they are needed at the 26
 //               neighbours by div n and div q), then every thread does its node: kappa_c = div n,
-//               F^s, F^p, F^nu (Eq. 8), pull-stream, moments, Hermite coefficient, regularized reconstruction, aligned
-//               store (Eqs. 6-7), u and r = D lap phi - kappa div q (Eq. 3).
-//               FUSED: u and r never leave the SM.  One plane behind the node update the block evaluates the advective
-//               WENO5 fluxes Phi_e = u_f WENO5(phi) (R12) through every face INSIDE its tile column
-//               (x faces: neighbour lane; y faces: shared memory; z faces: carried along the march) and writes
+//               F^s, F^p, F^nu, F^g (Eq. 8, R31), pull-stream, moments, Hermite coefficient, regularized reconstruction,
+//               aligned store (Eqs. 6-7), u and r = D lap phi - kappa div q (Eq. 3).
+//               MODE_FUSED: u and r never leave the SM.  One plane behind the node update the block evaluates the
+//               advective WENO5 fluxes Phi_e = u_f WENO5(phi) (R12) through every face INSIDE its tile
+//               column (x faces: neighbour lane; y faces: shared memory; z faces: carried along the march) and writes
 //               phi(t+1) = phi + r - sum_e (Phi_e(x) - Phi_e(x - e)) without the faces on the tile's seams, whose second
-//               velocity belongs to another block; the velocities on the seams go to three thin strips (2.6 B per node).
+//               velocity belongs to another block; the velocities on the seams go to three thin strips (2.75 B per node).
+//               The other modes reuse the march and the geometry: MODE_UNFUSED (u, r to HBM for k_advect: variant 1 and
+//               the SSP-RK3 stages), MODE_MOMENTS, MODE_DIAG, MODE_INIT (accLB_moments / diagnostics / init).
 //   k_seam      adds the fluxes through the seam faces (x = multiples of TX, y = multiples of TY, z = multiples of lz:
 //               5 % of all faces) to the cells on either side, from the strips and phi(t): one thread per face, one
 //               flux per face, added to one cell and subtracted from the other (atomics): sum phi is conserved to
 //               rounding (R12).
-//   FUSED = false + k_advect is the round-1 two-kernel form (u, r through HBM), kept as variant 2 for comparison:
-//   k_advect    the advective part of a8: phi+ = phi + (-sum_e (Phi_e(x) - Phi_e(x - e)) + r); every face flux is
-//               computed once per face (shared memory for x / y faces, a register carried along z for z faces).
+//   k_advect    the advective part of a8 as a kernel of its own (after k_lb_tp<MODE_UNFUSED>):
+//               phi+ = a base + b (phi + (-sum_e (Phi_e(x) - Phi_e(x - e)) + r)); every face flux is computed once per face
+//               (shared memory for x / y faces, a register carried along z for z faces).
 // Periodic boundaries are index wraps when the tiles are filled (PAPER.md:L114's halo exchange is not needed).
-// Staging: the 27 pulled populations of the next plane arrive by TMA (27 tiled cp.async.bulk.tensor box loads issued by
-// one thread, mbarrier completion) in tiles away from the y rim, by one cp.async per thread and population elsewhere; phi,
-// u, r planes arrive by cp.async one plane ahead.
+// Staging: FAST instances (tile-divisible boxes, fp64 storage): the 27 pulled populations of the next plane arrive by TMA
+// (27 tiled cp.async.bulk.tensor box loads, mbarrier completion; tiles on the periodic y rim row by row); otherwise one
+// cp.async per thread and population.  phi planes arrive by 16-byte cp.async one plane ahead.
 #pragma once
 
 #include <type_traits>
