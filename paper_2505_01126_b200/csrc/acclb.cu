@@ -532,13 +532,17 @@ static int launch_lb_tp(accLB_ctx* s, int c, int d, int kind, double* out_u, dou
   return ACCLB_OK;
 }
 
-// FAST (all tiles full, TMA pull) when the tensor maps exist and the tile shape divides the box; fp64 storage only.
+// FAST (all tiles full, TMA pull) when the tensor maps exist and the tile shape divides the box.
 template <int MODE>
 static int launch_lb_tp_any(accLB_ctx* s, int c, int d, int kind = KIND_LB_TP, double* out_u = nullptr,
                             double* out_r = nullptr, const double* in0 = nullptr, const double* in1 = nullptr) {
   if (MODE == MODE_UNFUSED) { out_u = s->u; out_r = s->r; }
-  if (s->prm.store_fp32) return launch_lb_tp<float, MODE, false>(s, c, d, kind, out_u, out_r, in0, in1);
-  if (MODE != MODE_INIT && s->tmap_ok) return launch_lb_tp<double, MODE, MODE != MODE_INIT>(s, c, d, kind, out_u, out_r, in0, in1);
+  constexpr bool CAN_FAST = MODE != MODE_INIT;
+  if (s->prm.store_fp32) {
+    if (CAN_FAST && s->tmap_ok) return launch_lb_tp<float, MODE, CAN_FAST>(s, c, d, kind, out_u, out_r, in0, in1);
+    return launch_lb_tp<float, MODE, false>(s, c, d, kind, out_u, out_r, in0, in1);
+  }
+  if (CAN_FAST && s->tmap_ok) return launch_lb_tp<double, MODE, CAN_FAST>(s, c, d, kind, out_u, out_r, in0, in1);
   return launch_lb_tp<double, MODE, false>(s, c, d, kind, out_u, out_r, in0, in1);
 }
 
@@ -626,18 +630,18 @@ static int make_tensor_maps(accLB_ctx* s) {
     cudaGetLastError();
     return 0;
   }
-  if (s->prm.store_fp32) return 0;  // measured: with 128-byte rows the per-thread cp.async pull is faster (9.5 vs 9.9 ms)
-  const size_t es = 8;
+  const size_t es = s->prm.store_fp32 ? 4 : 8;
+  const CUtensorMapDataType dt = s->prm.store_fp32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
   if (s->nx % LBT_TX != 0 || s->ny % LBT_TY != 0) return 0;  // FAST: every tile full
   const cuuint64_t dims[3] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny, (cuuint64_t)(s->prm.moment_storage ? 10 : 27) * s->nz};
   const cuuint64_t strides[2] = {(cuuint64_t)s->nx * es, (cuuint64_t)s->nx * s->ny * es};
   const cuuint32_t box[3] = {LBT_TX, LBT_TY, 1}, row[3] = {LBT_TX, 1, 1}, estr[3] = {1, 1, 1};
   for (int b = 0; b < 2; ++b) {
-    CUresult r = ((encode_t)fn)(&s->tmap[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, s->f[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    CUresult r = ((encode_t)fn)(&s->tmap[b], dt, 3, s->f[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return 0;
-    r = ((encode_t)fn)(&s->tmap_row[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, s->f[b], dims, strides, row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    r = ((encode_t)fn)(&s->tmap_row[b], dt, 3, s->f[b], dims, strides, row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return 0;
   }

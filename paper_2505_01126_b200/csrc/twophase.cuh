@@ -174,7 +174,7 @@ __device__ __forceinline__ double seam_face_flux(const Grid& G, const double* __
 // The 27 populations a thread pulls for plane z are fetched with TMA / cp.async into shared memory while
 // the block is still busy with plane z-1 and with the geometry of plane z: the HBM latency of the pull hides under the
 // fp64 work instead of stalling every warp at the top of the node update, and no register holds a load in flight.
-// FAST (fp64 storage, nx a multiple of TX, ny a multiple of TY, tensor maps available): every tile is full and pulls by
+// FAST (nx a multiple of TX, ny a multiple of TY, tensor maps available): every tile is full and pulls by
 // TMA; no thread is idle and no per-thread wrap tables are kept.  Otherwise every tile pulls with per-thread cp.async.
 // MODE: what a node does with its moments and its force -- the march, the staging and the geometry are the same:
 //   MODE_FUSED    the time step (default): collide + store, advection fused, seam strips            rows a1-a8
@@ -199,7 +199,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const __grid_constant__ CUtensorMap tmap_row, const double* __restrict__ in0, const double* __restrict__ in1) {
   constexpr bool FUSED = MODE == MODE_FUSED;
   constexpr bool PULL = MODE != MODE_INIT;  // the populations of the current state are needed
-  static_assert(!FAST || sizeof(ST) == 8, "the TMA pull is for fp64 storage");
+  constexpr int EC = 16 / (int)sizeof(ST);  // elements per 16-byte chunk: the edge elements of the TMA pull are fetched as aligned chunks
   static_assert(!(FAST && MODE == MODE_INIT), "the push of the initial state uses the per-thread wrap tables");
   using T = GeoTile<ST, TX, TY, FUSED>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
@@ -261,9 +261,9 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   }
   // three per-thread bases, one per c_ix, so that slot(i) is base + a compile-time offset
   ST* const sl_c = &S.fpop[0][ty * TX + tx];
-  // (FAST: the slab's tail holds, per tile row, the aligned pair (x0-2, x0-1) for c_ix = +1 / (x0+TX, x0+TX+1) for -1)
-  ST* const sl_p = tx == 0 ? &S.fpop[0][NT + (fast ? 2 * ty + 1 : ty)] : sl_c - 1;       // c_ix = +1: element x - 1
-  ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + (fast ? 2 * ty : ty)] : sl_c + 1;      // c_ix = -1: element x + 1
+  // (FAST: the slab's tail holds, per tile row, the aligned 16-byte chunk that ends at x0-1 (c_ix = +1) / starts at x0+TX (-1))
+  ST* const sl_p = tx == 0 ? &S.fpop[0][NT + (fast ? EC * ty + EC - 1 : ty)] : sl_c - 1;  // c_ix = +1: element x - 1
+  ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + (fast ? EC * ty : ty)] : sl_c + 1;       // c_ix = -1: element x + 1
   auto slot = [&](int i) -> ST* { return (cx_of(i) == 0 ? sl_c : cx_of(i) == 1 ? sl_p : sl_m) + i * T::SLAB; };
   // The TMA issue is spread over the block's warps (warp w issues boxes w, w + TY, ...): one thread issuing all 27 made
   // its warp arrive late at the next barrier in every iteration.  Thread 0 arms the mbarrier with the byte count.
@@ -299,14 +299,14 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     const int m = tx < 9 ? tx : tx - 9;
     const int e_i = 3 * m + (tx < 9 ? 2 : 0), cy = m % 3 - 1;
     e_off = (unsigned)e_i * plane + (unsigned)pmod(y - cy, G.ny) * (unsigned)G.nx +
-            (unsigned)(tx < 9 ? pmod(x0 - 2, G.nx) : pmod(x0 + TX, G.nx));
+            (unsigned)(tx < 9 ? pmod(x0 - EC, G.nx) : pmod(x0 + TX, G.nx));
   }
   auto prefetch_pull = [&](int z) {
     if (fast) {  // the boxes are on their way (after the block-wide hand-over)
       if (tx < 18) {
         const int m = tx < 9 ? tx : tx - 9;  // population 3 m + 2 (c_ix = +1) or 3 m (c_ix = -1), c_iz = m / 3 - 1
         const ST* sl = pop_slab(fin, G, m < 3 ? wrap_inc(z, G.nz) : m >= 6 ? wrap_dec(z, G.nz) : z);
-        cp_async_16(&S.fpop[3 * m + (tx < 9 ? 2 : 0)][NT + 2 * ty], sl + e_off);
+        cp_async_16(&S.fpop[3 * m + (tx < 9 ? 2 : 0)][NT + EC * ty], sl + e_off);
       }
       cp_async_commit();
       return;
