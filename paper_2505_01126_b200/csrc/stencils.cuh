@@ -60,45 +60,6 @@ __device__ __forceinline__ T* pop_slab(T* f, const Grid& G, int z) {
   return p;
 }
 
-// Lattice derivative along AX of a periodic field given through `val(dz, dy, dx)`.
-//   (1/cs2) sum_i w_i c_i,AX val(c_i) = (1/72) sum_{p,q in -1..1} W(p) W(q) (val(+1; p,q) - val(-1; p,q)), W = (1,4,1)
-template <int AX, class V>
-__device__ __forceinline__ double lattice_derivative(V val) {
-  double acc = 0.0;
-#pragma unroll
-  for (int p = -1; p <= 1; ++p)
-#pragma unroll
-    for (int q = -1; q <= 1; ++q) {
-      const double wgt = (p == 0 ? 4.0 : 1.0) * (q == 0 ? 4.0 : 1.0);
-      double d;
-      if (AX == 0) d = val(p, q, 1) - val(p, q, -1);        // (dz,dy) = (p,q)
-      else if (AX == 1) d = val(p, 1, q) - val(p, -1, q);   // (dz,dx) = (p,q)
-      else d = val(1, p, q) - val(-1, p, q);                // (dy,dx) = (p,q)
-      acc = fma(wgt, d, acc);
-    }
-  return acc * (1.0 / 72.0);
-}
-
-// Gradient and Laplacian of one scalar whose 27 neighbourhood values are in v[dz+1][dy+1][dx+1].
-__device__ __forceinline__ void gradient27(const double (&v)[3][3][3], double (&g)[3]) {
-  g[0] = lattice_derivative<0>([&](int dz, int dy, int dx) { return v[dz + 1][dy + 1][dx + 1]; });
-  g[1] = lattice_derivative<1>([&](int dz, int dy, int dx) { return v[dz + 1][dy + 1][dx + 1]; });
-  g[2] = lattice_derivative<2>([&](int dz, int dy, int dx) { return v[dz + 1][dy + 1][dx + 1]; });
-}
-
-__device__ __forceinline__ double laplacian27(const double (&v)[3][3][3]) {
-  // (2/cs2) sum_i w_i (v_i - v_0) = 6 (sum_i w_i v_i - v_0), w_i = W W W / 216
-  double acc = 0.0;
-#pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int b = 0; b < 3; ++b) {
-      const double row = v[a][b][0] + 4.0 * v[a][b][1] + v[a][b][2];
-      acc = fma((a == 1 ? 4.0 : 1.0) * (b == 1 ? 4.0 : 1.0), row, acc);
-    }
-  return 6.0 * (acc * (1.0 / 216.0) - v[1][1][1]);
-}
-
 // sqrt(s) for s >= 0: hardware reciprocal-square-root seed, two Newton steps on y ~ 1/sqrt(s), then s y with one residual
 // correction; relative error ~1e-16, a fixed instruction sequence without the library routine's special-case call.
 // s = 0 gives 0 (the seed is taken of max(s, 1e-300); below that the result is only needed to be << 1e-12, R17).

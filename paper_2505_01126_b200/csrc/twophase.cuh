@@ -38,20 +38,6 @@ __device__ __forceinline__ int pmod(int a, int n) {
   return r < 0 ? r + n : r;
 }
 
-// (2/cs2) sum_i w_i (Psi(x + c_i) - Psi(x)) through an accessor val(dz, dy, dx); PAPER.md:L104 as repaired by R7.
-template <class V>
-__device__ __forceinline__ double lattice_laplacian(V val) {
-  double acc = 0.0;
-#pragma unroll
-  for (int a = -1; a <= 1; ++a)
-#pragma unroll
-    for (int b = -1; b <= 1; ++b) {
-      const double row = val(a, b, -1) + 4.0 * val(a, b, 0) + val(a, b, 1);
-      acc = fma((a == 0 ? 4.0 : 1.0) * (b == 0 ? 4.0 : 1.0), row, acc);
-    }
-  return 6.0 * (acc * (1.0 / 216.0) - val(0, 0, 0));
-}
-
 // cp.async (LDGSTS) of one population from global memory into the issuing thread's own shared-memory slot.  Default L2
 // policy on purpose: with an evict-first hint the 32-byte sectors that the x-shifted pulls of two neighbouring tiles share
 // were evicted between the two reads (ncu: 36.0 GB read per 512^3 step with the hint, 30.9 GB without; ideal 30.1 GB).
