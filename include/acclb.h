@@ -70,6 +70,14 @@ typedef struct {
   int moment_storage; /* 1: the state is the paper's ten macroscopic fields (p*, u, a) per node instead of 27 populations
                          (160 B instead of 432 B moved per node and step; same results to rounding); single component,
                          fp64 only (two_phase = 0, store_fp32 = 0) */
+  /* z-slab decomposition over several GPUs (PAPER.md:L114 halo exchange, L126 slab weak scaling) */
+  int halo_z;    /* 0: the box is periodic in z (one GPU holds the whole domain).  h > 0: the box is one z-slab of a larger
+                    periodic domain: its first and last h planes are HALO planes, copies of the neighbouring slabs' boundary
+                    planes that the caller refreshes after every step (accLB_halo_chunks); only planes [h, nz - h) are this
+                    slab's own nodes.  Needs h >= 3 for two_phase (WENO5 radius 3, R12), h >= 1 otherwise, nz >= 3 h;
+                    forward Euler, population storage only (phi_integrator = 0, moment_storage = 0).                     */
+  int z_origin;  /* halo_z > 0: global z coordinate of local plane 0 (may be negative: periodic), for the body force R20   */
+  int nz_global; /* halo_z > 0: planes of the whole domain (the period of the body force along z)                          */
 } accLB_params;
 
 /* Bytes of device workspace accLB_create needs for this grid and these parameters; 0 on invalid arguments
@@ -97,6 +105,7 @@ int accLB_moments(accLB_ctx* ctx, double* rho, double* u, double* phi);
 /* Diagnostics of the current state (R21) into out[0..ACCLB_NDIAG-1] (HOST pointer, n_out >= ACCLB_NDIAG):
  *   0 KE = <rho(phi) |u|^2 / 2>      1 dissipation = <nu a:a / (2 cs^4 tau^2)>
  *   2 sum phi   3 sum p*   4..6 sum_x sum_i f_i c_i   7 max |u|   8 step count.
+ * With halo_z = h > 0 the sums, means and the maximum run over the slab's own planes [h, nz - h) only.
  * Warp-shuffle + one atomic per block and quantity.  Synchronises the stream.  ACCLB_ENUMERIC if non-finite. */
 int accLB_diagnostics(accLB_ctx* ctx, double* out, int n_out);
 
@@ -129,6 +138,33 @@ int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
  * kept so that bench.py / ncu can compare fused and unfused on identical inputs.  Results are
  * identical to rounding.  Single-phase contexts and phi_integrator = 1 have one path.  ACCLB_EINVAL for an unknown variant. */
 int accLB_set_variant(accLB_ctx* ctx, int variant);
+
+/* ---- z-slab decomposition ("halo regions ... exchanged between neighbouring subdomains",
+ * L126 slab weak scaling).  A context created with params.halo_z = h > 0 advances a box whose first and last h planes are
+ * halo planes.  One step leaves its own planes [h, nz - h) correct provided that, before the step, the halo planes hold
+ * the neighbours' current state in the parts listed below; everything else in the halo planes is scratch (it is advanced
+ * like the rest of the box with a periodic wrap that means nothing, and is never read by a node of [h, nz - h)).
+ *   populations (stored post-collision, pulled at the next step: f_i(x, t+1) = f*_i(x - c_i, t)):
+ *     low side   plane h-1: c_z >= 0 (i = 9..26; c_z = +1 streams into plane h, c_z = 0 completes the moments of plane
+ *                h-1 whose velocity u enters the phi flux through the face between h-1 and h);  plane h-2: c_z = +1 only
+ *                (i = 18..26; pulled by plane h-1).  Single component: plane h-1, c_z = +1 only.
+ *     high side  mirrored: plane nz-h: i = 0..17, plane nz-h+1: i = 0..8.
+ *   phi: all h halo planes of either side (WENO5 radius 3; curvature of plane h-1 reaches phi of plane h-3).
+ * accLB_halo_chunks lists, for the CURRENT state buffers (they alternate from step to step: call it after every step), the
+ * contiguous DEVICE byte ranges to send to and to receive from the two z-neighbours: out[j] for j < return value <= cap.
+ *   side  -1: the neighbour that owns the planes below this slab, +1: above.    dir  0: send (read), 1: receive (written).
+ * The k-th send range towards a side pairs with the k-th receive range from the opposite side of that neighbour, and has the
+ * same length.  full != 0 lists every population of all h halo planes instead of the minimal set (3 x the bytes; then
+ * nothing in the halo planes is scratch).  The copy itself is the caller's (NCCL send/recv, peer copies).
+ * Returns the number of ranges, or a negative error (ACCLB_EINVAL: NULL, halo_z = 0, cap too small). */
+typedef struct {
+  void* ptr;    /* DEVICE address inside the workspace */
+  size_t bytes;
+  int side;     /* -1 | +1 */
+  int dir;      /* 0 send | 1 receive */
+} accLB_halo_chunk;
+#define ACCLB_MAX_HALO_CHUNKS 16
+int accLB_halo_chunks(accLB_ctx* ctx, int full, accLB_halo_chunk* out, int cap);
 
 /* Free the context (host memory only; the workspace stays the caller's). */
 int accLB_destroy(accLB_ctx* ctx);

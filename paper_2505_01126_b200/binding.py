@@ -22,7 +22,7 @@ ERRORS = {0: "ACCLB_OK", -1: "ACCLB_EINVAL", -2: "ACCLB_EWORKSPACE", -3: "ACCLB_
 
 SYMBOLS = ("accLB_workspace_bytes", "accLB_create", "accLB_init", "accLB_step", "accLB_moments",
            "accLB_diagnostics", "accLB_run_host", "accLB_launch_count", "accLB_profile",
-           "accLB_profile_read", "accLB_set_variant", "accLB_destroy",
+           "accLB_profile_read", "accLB_set_variant", "accLB_halo_chunks", "accLB_destroy",
            "accLB_last_error", "accLB_stats_increments", "accLB_stats_pdf", "accLB_stats_spectrum")
 
 
@@ -38,7 +38,16 @@ class Params(C.Structure):
         ("device", C.c_int), ("stream", C.c_void_p),
         ("gravity", C.c_double * 3), ("rho_ref", C.c_double), ("phi_integrator", C.c_int),
         ("moment_storage", C.c_int),
+        ("halo_z", C.c_int), ("z_origin", C.c_int), ("nz_global", C.c_int),
     ]
+
+
+class HaloChunk(C.Structure):
+    """Mirror of ``accLB_halo_chunk``."""
+    _fields_ = [("ptr", C.c_void_p), ("bytes", C.c_size_t), ("side", C.c_int), ("dir", C.c_int)]
+
+
+MAX_HALO_CHUNKS = 16
 
 
 class AccLBError(RuntimeError):
@@ -73,6 +82,7 @@ def load():
     L.accLB_profile.argtypes = [C.c_void_p, C.c_int]
     L.accLB_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
     L.accLB_set_variant.argtypes = [C.c_void_p, C.c_int]
+    L.accLB_halo_chunks.argtypes = [C.c_void_p, C.c_int, C.POINTER(HaloChunk), C.c_int]
     L.accLB_destroy.argtypes = [C.c_void_p]
     L.accLB_last_error.restype = C.c_char_p
     L.accLB_stats_increments.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_double), _dp,
@@ -92,10 +102,10 @@ def _check(code):
 
 def make_params(*, tau, two_phase=0, rho_l=1.0, rho_g=1.0, sigma=0.0, mobility=0.0, width=4.0, force_type=0,
                 force_amp=0.0, force_k=1, store_fp32=0, host_staging=0, device=0, stream=None,
-                gravity=(0.0, 0.0, 0.0), rho_ref=0.0, phi_rk3=0, moment_storage=0):
+                gravity=(0.0, 0.0, 0.0), rho_ref=0.0, phi_rk3=0, moment_storage=0, halo_z=0, z_origin=0, nz_global=0):
     return Params(tau, int(two_phase), rho_l, rho_g, sigma, mobility, width, int(force_type), force_amp, int(force_k),
                   int(store_fp32), int(host_staging), int(device), stream, (C.c_double * 3)(*gravity), rho_ref,
-                  int(phi_rk3), int(moment_storage))
+                  int(phi_rk3), int(moment_storage), int(halo_z), int(z_origin), int(nz_global))
 
 
 def workspace_bytes(nx, ny, nz, params):
@@ -206,6 +216,21 @@ class AccLB:
 
     def set_variant(self, v):
         _check(load().accLB_set_variant(self._h, int(v)))
+
+    def halo_chunks(self, full=False):
+        """The halo exchange of a z-slab context for its CURRENT buffers: a list of (view, side, dir), `view` a uint8 view
+        into the workspace (no copy), side -1 / +1 the z-neighbour, dir 0 = send, 1 = receive (include/acclb.h)."""
+        arr = (HaloChunk * MAX_HALO_CHUNKS)()
+        n = load().accLB_halo_chunks(self._h, int(bool(full)), arr, MAX_HALO_CHUNKS)
+        if n < 0:
+            _check(n)
+        base = self.workspace.data_ptr()
+        out = []
+        for c in arr[:n]:
+            off = c.ptr - base
+            assert 0 <= off and off + c.bytes <= self.workspace.numel()
+            out.append((self.workspace[off:off + c.bytes], c.side, c.dir))
+        return out
 
     @property
     def launch_count(self):

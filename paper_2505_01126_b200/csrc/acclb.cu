@@ -43,6 +43,7 @@ struct KP {
   double nu, eps_pref;        // nu, nu / (2 cs4 tau^2) (R21)
   double grav[3], rho_ref;    // buoyancy F^g = (rho - rho_ref) g       PAPER.md:L193, L203 (R31)
   int buoyant;                // g != 0
+  int zlo, zhi;               // diagnostics run over planes [zlo, zhi): all of them, or a slab's own planes (halo_z)
 };
 
 // population storage: fp64, or fp32 deviation from the lattice weight (R22)
@@ -291,6 +292,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_diagnostics(KP P, const ST* __
     const int x = (int)(k % (unsigned)G.nx);
     const unsigned yz = k / (unsigned)G.nx;
     const int y = (int)(yz % (unsigned)G.ny), z = (int)(yz / (unsigned)G.ny);
+    if (z < P.zlo || z >= P.zhi) continue;  // halo planes of a z-slab
     Nbr nb;
     make_nbr(G, x, y, z, nb);
     double f[Q];
@@ -458,6 +460,12 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
   if (p->phi_integrator < 0 || p->phi_integrator > 1) return false;
   if (p->moment_storage < 0 || p->moment_storage > 1) return false;
   if (p->moment_storage && (p->two_phase || p->store_fp32)) return false;  // single-phase fp64 only
+  if (p->halo_z < 0) return false;
+  if (p->halo_z > 0) {  // one z-slab of a larger periodic domain
+    if (p->phi_integrator != 0 || p->moment_storage) return false;
+    if (p->halo_z < (p->two_phase ? 3 : 1) || nz < 3 * p->halo_z) return false;
+    if (p->nz_global < nz - 2 * p->halo_z) return false;
+  }
   if (p->two_phase) {
     if (!(p->rho_l > 0.0) || !(p->rho_g > 0.0) || !(p->width > 0.0) || !(p->mobility >= 0.0)) return false;
   }
@@ -718,6 +726,8 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   k.buoyant = p->gravity[0] != 0.0 || p->gravity[1] != 0.0 || p->gravity[2] != 0.0;
   k.nu = (p->tau - 0.5) / 3.0;
   k.eps_pref = k.nu / (2.0 * (1.0 / 9.0) * p->tau * p->tau);
+  k.zlo = p->halo_z;
+  k.zhi = nz - p->halo_z;
 
   // R20: per-axis sin/cos tables, libm on the host, k = 2 pi force_k / N, integer node coordinates
   std::vector<double> t((size_t)2 * (nx + ny + nz));
@@ -725,9 +735,17 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   const int dims[3] = {nx, ny, nz};
   size_t o = 0;
   for (int ax = 0; ax < 3; ++ax) {
-    const double kk = two_pi * p->force_k / dims[ax];
-    for (int j = 0; j < dims[ax]; ++j) t[o + j] = sin(kk * (double)j);
-    for (int j = 0; j < dims[ax]; ++j) t[o + dims[ax] + j] = cos(kk * (double)j);
+    // a z-slab (halo_z > 0) takes the table entries of its own planes out of the whole domain's table: the global
+    // coordinate is reduced into [0, nz_global) first so that every slab evaluates sin / cos of the same arguments
+    const bool slab = ax == 2 && p->halo_z > 0;
+    const int period = slab ? p->nz_global : dims[ax];
+    const double kk = two_pi * p->force_k / period;
+    for (int j = 0; j < dims[ax]; ++j) {
+      int g = j;
+      if (slab) g = ((p->z_origin + j) % period + period) % period;
+      t[o + j] = sin(kk * (double)g);
+      t[o + dims[ax] + j] = cos(kk * (double)g);
+    }
     o += (size_t)2 * dims[ax];
   }
   cudaError_t e = cudaMemcpyAsync(s->tabs, t.data(), t.size() * 8, cudaMemcpyHostToDevice, s->stream);
@@ -862,7 +880,7 @@ int accLB_diagnostics(accLB_ctx* s, double* out, int n_out) {
   double h[8];
   CK(cudaMemcpyAsync(h, s->acc, sizeof h, cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
-  const double inv_n = 1.0 / (double)s->n;
+  const double inv_n = 1.0 / ((double)s->nx * s->ny * (s->kp.zhi - s->kp.zlo));
   out[0] = h[0] * inv_n;
   out[1] = h[1] * inv_n;
   out[2] = h[2];
@@ -944,6 +962,67 @@ int accLB_profile_read(accLB_ctx* s, double* ms, long long* count, int n) {
     s->folded_count[k] = 0;
   }
   return ACCLB_OK;
+}
+
+// The byte ranges of the halo exchange of a z-slab (include/acclb.h): whole [ny][nx] planes of consecutive populations of
+// one z plane are contiguous in the [z][i][y][x] layout, so every item is one range.
+int accLB_halo_chunks(accLB_ctx* s, int full, accLB_halo_chunk* out, int cap) {
+  if (!s || !out) return fail(ACCLB_EINVAL, "accLB_halo_chunks: NULL argument");
+  const int h = s->prm.halo_z;
+  if (h <= 0) return fail(ACCLB_EINVAL, "accLB_halo_chunks: the context is not a z-slab (halo_z = 0)");
+  const size_t plane = (size_t)s->nx * s->ny;
+  const size_t es = s->prm.store_fp32 ? 4 : 8;
+  char* f = (char*)s->f[s->cur];
+  const int nz = s->nz;
+  int n = 0;
+  bool overflow = false;
+  auto add = [&](void* ptr, size_t bytes, int side, int dir) {
+    if (n >= cap) { overflow = true; return; }
+    out[n].ptr = ptr; out[n].bytes = bytes; out[n].side = side; out[n].dir = dir;
+    ++n;
+  };
+  // populations i0 .. i1-1 of plane z
+  auto pops = [&](int z, int i0, int i1, int side, int dir) {
+    add(f + ((size_t)z * 27 + i0) * plane * es, (size_t)(i1 - i0) * plane * es, side, dir);
+  };
+  auto phis = [&](int z0, int side, int dir) {
+    if (s->prm.two_phase) add(s->phi[s->cur] + (size_t)z0 * plane, (size_t)h * plane * 8, side, dir);
+  };
+  for (int dir = 0; dir < 2; ++dir) {
+    // dir 0: my own boundary planes, sent; dir 1: my halo planes, received.  The planes sent DOWN are the ones the lower
+    // neighbour receives into its HIGH halo, and the other way round: the send list towards a side mirrors the receive
+    // list from the other side.
+    if (full) {
+      // low end: halo planes [0, h) received from below | own planes [h, 2h) sent down
+      pops(dir ? 0 : h, 0, 27 * h, -1, dir);
+      phis(dir ? 0 : h, -1, dir);
+      pops(dir ? nz - h : nz - 2 * h, 0, 27 * h, +1, dir);
+      phis(dir ? nz - h : nz - 2 * h, +1, dir);
+      continue;
+    }
+    const bool tp = s->prm.two_phase != 0;
+    if (dir == 1) {
+      // received from below: plane h-1 (c_z >= 0, or c_z = +1 single component), plane h-2 (c_z = +1)
+      pops(h - 1, tp ? 9 : 18, 27, -1, 1);
+      if (tp) pops(h - 2, 18, 27, -1, 1);
+      phis(0, -1, 1);
+      // received from above: plane nz-h (c_z <= 0 | c_z = -1), plane nz-h+1 (c_z = -1)
+      pops(nz - h, 0, tp ? 18 : 9, +1, 1);
+      if (tp) pops(nz - h + 1, 0, 9, +1, 1);
+      phis(nz - h, +1, 1);
+    } else {
+      // sent down (the lower neighbour's "received from above"): my planes h, h+1
+      pops(h, 0, tp ? 18 : 9, -1, 0);
+      if (tp) pops(h + 1, 0, 9, -1, 0);
+      phis(h, -1, 0);
+      // sent up (the upper neighbour's "received from below"): my planes nz-h-1, nz-h-2
+      pops(nz - h - 1, tp ? 9 : 18, 27, +1, 0);
+      if (tp) pops(nz - h - 2, 18, 27, +1, 0);
+      phis(nz - 2 * h, +1, 0);
+    }
+  }
+  if (overflow) return fail(ACCLB_EINVAL, "accLB_halo_chunks: cap = %d is too small (ACCLB_MAX_HALO_CHUNKS)", cap);
+  return n;
 }
 
 int accLB_destroy(accLB_ctx* s) {

@@ -572,7 +572,8 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         if (MODE == MODE_MOMENTS && rout) rout[k] = M.p;
       }
       if (MODE == MODE_FUSED || MODE == MODE_UNFUSED) collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
-      if (MODE == MODE_DIAG) {  // R21: rho |u|^2 / 2, nu a:a / (2 cs4 tau^2), phi, p*, m, max |u|
+      if (MODE == MODE_DIAG && z >= P.zlo && z < P.zhi) {  // R21: rho |u|^2 / 2, nu a:a / (2 cs4 tau^2), phi, p*, m, max |u|;
+                                                            // a z-slab sums its own planes only
         double a6[6];
         hermite_coeff(M, u, A, a6);
         const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
