@@ -5,6 +5,7 @@
     python bench.py --impl reference [--steps K] [--warmup W]        # the CPU oracle as it stands, ONE JSON line
     torchrun --nproc-per-node N ... bench.py --gpus N ...            # N independent replicas ("replicas only")
     python bench.py --sweep [--sweep-out FILE]                       # BASELINE config 5 table (several JSON lines)
+    [torchrun ...] bench.py --slabs --gpus N ...                     # one domain in N z-slabs with halo exchange (8(f) #3)
 
 A "step" is one pass of the whole hot path (rows a1-a8: pull-stream, moments, phase geometry,
 forces, velocity, Hermite coefficient, regularized reconstruction, conservative Allen-Cahn update) over one lattice.
@@ -416,6 +417,88 @@ def run_cuda(args):
         torch.distributed.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------------ z-slabs (8(f) #3)
+def run_slabs(args):
+    """`--slabs`: ONE periodic domain n x n x (n * N) cut into N z-slabs, one per rank / GPU (the shape of the paper's weak
+    scaling, PAPER.md:L126), halo exchange after every step inside the timed region (NCCL send / recv between the ranks;
+    with N = 1 the rank is its own neighbour and the exchange is device copies).  The fields are the n^3 workload repeated
+    along z.  Not the driver's line: `python bench.py --gpus N` without --slabs stays "replicas only"."""
+    import numpy as np
+    import torch
+
+    from paper_2505_01126_b200 import build as _build, slabs
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA arm has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    barrier = lambda: None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+        barrier = dist.barrier
+    if rank == 0:
+        _build.build()
+    barrier()
+    n = args.n
+    cfg = make_workload(args.workload, n)
+    two_phase = bool(cfg["params"]["two_phase"])
+    part = slabs.SlabAccLB(n, n, n * world, rank=rank, world=world, device=local_rank, store_fp32=int(args.fp32), **cfg["params"])
+    sl = part.slab
+    planes = np.arange(sl.z_origin, sl.z_origin + sl.nz_local) % n   # the n^3 fields repeat along z
+    loc = {k: torch.from_numpy(np.ascontiguousarray(np.take(cfg[k], planes, axis=1 if k == "u" else 0))).to(dev)
+           for k in ("rho", "u", "phi") if cfg[k] is not None}
+    part.init(loc["rho"], loc["u"], loc.get("phi"))
+    part.step(args.warmup)
+    torch.cuda.synchronize(dev)
+    d0 = part.diagnostics()
+    stream = torch.cuda.current_stream(dev)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+    launches0 = part.sim.launch_count
+    barrier()
+    torch.cuda.synchronize(dev)
+    with ClockSampler(local_rank) as clk:
+        ev[0].record(stream)
+        for t in range(args.steps):
+            part.sim.step(1)
+            ev[2 * t + 1].record(stream)
+            part.exchange()
+            ev[2 * t + 2].record(stream)
+        torch.cuda.synchronize(dev)
+    barrier()
+    launches = part.sim.launch_count - launches0  # the copies / NCCL kernels of the exchange are not counted
+    ms = ev[0].elapsed_time(ev[-1])
+    ms_x = sum(ev[2 * t + 1].elapsed_time(ev[2 * t + 2]) for t in range(args.steps))
+    d1 = part.diagnostics()
+    ms, ms_x = max_over_ranks([ms, ms_x], f"cuda:{local_rank}" if world > 1 else None)
+    if rank == 0:
+        own = n ** 3
+        bpl = step_bytes_per_lup(bool(args.fp32), two_phase)
+        peak, how = hbm_peak()
+        value = world * own * args.steps / (ms * 1e-3) / 1e9
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload} {n} x {n} x {n * world} {'two' if two_phase else 'single'}-phase, one periodic "
+                                   f"domain in {world} z-slab(s) of {n} planes + {sl.halo} halo planes per side; the {n}^3 fields "
+                                   "repeated along z; " + WORKLOADS[args.workload][1],
+                       "parallelism": f"z-slabs x{world}, one halo exchange per step ("
+                                      + ("NCCL send/recv" if world > 1 else "the rank is its own neighbour: device copies") + ")",
+                       "halo_bytes_sent_per_rank_and_step": part.halo_bytes_per_step(),
+                       "lups_per_step": world * own, "planes_computed_per_rank": sl.nz_local},
+            "exchange_ms_per_step": ms_x / args.steps, "clocks": clk.summary(),
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "scope": "whole step incl. halo exchange, own planes only", "unit": "GB/s", "peak": peak * world,
+                         "peak_source": how, "achieved": value * bpl, "frac": value * bpl / (peak * world), "traffic": None},
+            "diagnostics": {"before": d0, "after": d1}}), flush=True)
+    part.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
 # ------------------------------------------------------------------------------------------------------ config 5 sweep
 def run_sweep(args):
     """BASELINE config 5: N in {64,...,512}, single- and two-phase, fp64 and fp32 population storage; 200 timed steps
@@ -457,6 +540,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-single", action="store_true", help="skip the single_phase leg of a two-phase run")
+    ap.add_argument("--slabs", action="store_true", help="one domain n x n x (n N) in N z-slabs with halo exchange (SURVEY 8(f) #3) "
+                                                         "instead of N independent replicas")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--sweep-sizes", default="64,128,256,384,512")
     ap.add_argument("--sweep-out", default=None)
@@ -467,6 +552,8 @@ def main():
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.slabs:
+        return run_slabs(args)
     return run_cuda(args)
 
 
