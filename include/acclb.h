@@ -21,7 +21,8 @@
  *     accLB_workspace_bytes() bytes, 256-byte aligned, that must outlive the context.  It never frees caller
  *     memory.  All work is enqueued on params.stream of device params.device.
  *   - Return value 0 = ACCLB_OK, negative = error; accLB_last_error() gives the text (thread-local).
- *   - A context is not thread-safe; distinct contexts are independent ("replicas only" across GPUs).
+ *   - A context is not thread-safe; distinct contexts are independent (replicas across GPUs; or z-slabs of one domain
+ *     whose halo planes the caller exchanges between steps, see accLB_halo_chunks).
  *   - There is no CPU fallback: every entry point needs a CUDA device.
  */
 #ifndef ACCLB_H
