@@ -98,7 +98,8 @@ struct GeoTile {
   // tx - c_ix of its row; the one element per row that lies outside the box (x0 - 1 for c_ix = +1, x0 + TX for c_ix = -1)
   // is fetched by the edge lane itself with an 8-byte cp.async into the tail of the slab.
   // One slab per population: the box, then the TY edge elements, padded to a multiple of 128 bytes (TMA destination).
-  static constexpr int SLAB = TX * TY + 128 / (int)sizeof(ST);
+  static constexpr int TAIL_BYTES = 16 * TY <= 128 ? 128 : (16 * TY + 127) / 128 * 128;
+  static constexpr int SLAB = TX * TY + TAIL_BYTES / (int)sizeof(ST);
   alignas(128) ST fpop[Q][SLAB];
   unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
@@ -279,7 +280,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   // FAST: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
   // c_ix = -1) are fetched by lanes 0..17 of the row's warp, one 16-byte cp.async each (the aligned pair that holds the
   // element), into the tail of the slabs
-  static_assert(sizeof(ST) == 8 || TY * 16 <= 128, "edge pairs fit the slab tail");
+  static_assert(TY * 16 <= T::TAIL_BYTES, "edge chunks fit the slab tail");
   unsigned e_off = 0;  // i * plane + row + column of this lane's edge pair
   if (fast && tx < 18) {
     const int m = tx < 9 ? tx : tx - 9;
