@@ -128,16 +128,18 @@ long long accLB_launch_count(const accLB_ctx* ctx);
  * k_lb_tp in its init / moments / diagnostics mode for two-phase contexts), 6 k_lb_tp (the tiled two-phase step: LB +
  * geometry + advection), 7 k_seam (advective fluxes through the faces between its tile columns), 8 k_advect (variant 1
  * and the Runge-Kutta stages), 9 k_geom_r (D lap phi - kappa div q of a Runge-Kutta stage field), 10 k_mr_step (the single-phase step on the ten
- * macroscopic fields, moment_storage = 1); 0 and 2 are unused.
+ * macroscopic fields, moment_storage = 1), 11 k_lb_tp in its Runge-Kutta stage mode (phi_integrator = 1); 0 and 2 are unused.
  * This is how bench.py measures kernel durations inside the timed region. */
-#define ACCLB_NKERNELS 11
+#define ACCLB_NKERNELS 12
 int accLB_profile(accLB_ctx* ctx, int enable);
 int accLB_profile_read(accLB_ctx* ctx, double* ms, long long* count, int n);
 
 /* Select the kernel variant of the forward-Euler two-phase step: 0 = default (k_lb_tp fused with the advection + k_seam);
  * 1 = the unfused form, u(t) and r through HBM (k_lb_tp unfused + k_advect: the path the SSP-RK3 integrator runs on),
  * kept so that bench.py / ncu can compare fused and unfused on identical inputs.  Results are
- * identical to rounding.  Single-phase contexts and phi_integrator = 1 have one path.  ACCLB_EINVAL for an unknown variant. */
+ * identical to rounding.  With phi_integrator = 1: 0 = the fused step is the first Runge-Kutta stage (it also writes u(t)) and
+ * the two later stages run in the same tiled kernel without its LB half, each followed by k_seam; 1 = k_lb_tp unfused, then
+ * k_advect / k_geom_r per stage.  Single-phase contexts have one path.  ACCLB_EINVAL for an unknown variant. */
 int accLB_set_variant(accLB_ctx* ctx, int variant);
 
 /* ---- z-slab decomposition ("halo regions ... exchanged between neighbouring subdomains",

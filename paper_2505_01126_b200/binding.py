@@ -14,9 +14,9 @@ LIB_PATH = _PKG / "libacclb.so"
 HEADER = _PKG.parent / "include" / "acclb.h"
 
 NDIAG = 9
-NKERNELS = 11
+NKERNELS = 12
 KERNEL_NAMES = ("unused0", "k_lb", "unused2", "k_init", "k_moments", "k_diagnostics", "k_lb_tp", "k_seam",
-                "k_advect", "k_geom_r", "k_mr_step")
+                "k_advect", "k_geom_r", "k_mr_step", "k_lb_tp_stage")
 DIAG_NAMES = ("ke", "dissipation", "sum_phi", "sum_pstar", "sum_mx", "sum_my", "sum_mz", "umax", "step")
 ERRORS = {0: "ACCLB_OK", -1: "ACCLB_EINVAL", -2: "ACCLB_EWORKSPACE", -3: "ACCLB_ECUDA", -4: "ACCLB_ENUMERIC"}
 

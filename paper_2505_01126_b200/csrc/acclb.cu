@@ -6,9 +6,10 @@
 //   two-phase      k_lb_tp<MODE_FUSED> + k_seam (twophase.cuh): the same plus phase geometry, forces (a3, a4) and the
 //                  conservative Allen-Cahn update (a8) on shared-memory tiles marching along z, TMA / cp.async staging;
 //                  u and r never written to HBM                                        PAPER.md:L61-67 (Eq. 3), L100-104 (Eq. 8)
-//                  phi_integrator = 1 (SSP-RK3, R32): k_lb_tp<MODE_UNFUSED> + k_advect stages + k_geom_r (phase_rk.cuh);
-//                  variant 1 = the forward-Euler form of that unfused path (k_lb_tp<MODE_UNFUSED> + k_advect), kept so that
-//                  bench.py / ncu can compare fused and unfused on identical inputs.
+//                  phi_integrator = 1 (SSP-RK3, R32): k_lb_tp<MODE_FUSED_U> (the step + first stage, u(t) written out) +
+//                  k_seam, then twice k_lb_tp<MODE_STAGE> + k_seam<SCALED> (the same tiles without the LB half);
+//                  variant 1 = the unfused forms (k_lb_tp<MODE_UNFUSED> + k_advect; RK3: + k_geom_r (phase_rk.cuh) and
+//                  k_advect per stage), kept so that bench.py / ncu can compare fused and unfused on identical inputs.
 //   init, moments, diagnostics of a two-phase context are modes of the same tiled kernel.
 // State: post-collision, not yet streamed populations f*_i(x) in SoA [z][i][y][x], double-buffered (A/B), so the
 // pull f_i(x,t) = f*_i(x - c_i, t-1) reads shifted rows and every store is aligned; phi double-buffered.
@@ -44,6 +45,7 @@ struct KP {
   double grav[3], rho_ref;    // buoyancy F^g = (rho - rho_ref) g       PAPER.md:L193, L203 (R31)
   int buoyant;                // g != 0
   int zlo, zhi;               // diagnostics run over planes [zlo, zhi): all of them, or a slab's own planes (halo_z)
+  double rk_a, rk_b;          // Shu-Osher coefficients of the Runge-Kutta stage being launched (k_lb_tp<MODE_STAGE>, k_seam)
 };
 
 // population storage: fp64, or fp32 deviation from the lattice weight (R22)
@@ -435,7 +437,7 @@ struct LaunchScope {
   }
 };
 enum { KIND_LB = 1, KIND_INIT = 3, KIND_MOMENTS = 4, KIND_DIAG = 5, KIND_LB_TP = 6,
-       KIND_SEAM = 7, KIND_ADVECT = 8, KIND_GEOM = 9, KIND_MR = 10 };
+       KIND_SEAM = 7, KIND_ADVECT = 8, KIND_GEOM = 9, KIND_MR = 10, KIND_STAGE = 11 };
 
 static thread_local char g_err[512] = "";
 
@@ -473,6 +475,7 @@ static bool valid_args(int nx, int ny, int nz, const accLB_params* p) {
 }
 
 // Tile shapes of the two-phase kernels.
+constexpr int STAGE_MINB = 3;  // k_lb_tp<MODE_STAGE> holds no population landing zone: three blocks per SM
 constexpr int LBT_TX = 32, LBT_TY = 8, LBT_MINB = 2;  // (32 x 16 tiles, one 512-thread block per SM: measured 11.17 vs 10.52 ms at 512^3)
 constexpr int ADV_TX = 32, ADV_TY = 8;
 
@@ -522,11 +525,13 @@ static unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threa
 
 // One launch of the tiled two-phase kernel in the given MODE (twophase.cuh) on the state f[c], phi[c]; f[d], phi[d] are the
 // targets of a step.  out_u / out_r / in0 / in1: see the MODE list.
+// phi_in / phi_out (default: phi[c] / phi[d]) let a Runge-Kutta stage run on the stage fields.
 template <typename ST, int MODE, bool FAST>
 static int launch_lb_tp(accLB_ctx* s, int c, int d, int kind, double* out_u, double* out_r, const double* in0,
-                        const double* in1) {
-  using T = GeoTile<ST, LBT_TX, LBT_TY, MODE == MODE_FUSED>;
-  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, LBT_MINB, MODE, FAST>;
+                        const double* in1, const double* phi_in = nullptr, double* phi_out = nullptr) {
+  constexpr bool STAGE = MODE == MODE_STAGE;
+  using T = GeoTile<ST, LBT_TX, LBT_TY, MODE == MODE_FUSED || MODE == MODE_FUSED_U || STAGE, !STAGE>;
+  auto kern = k_lb_tp<ST, LBT_TX, LBT_TY, STAGE ? STAGE_MINB : LBT_MINB, MODE, FAST>;
   static thread_local int configured_device = -1;
   if (configured_device != s->prm.device) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(T)));
@@ -535,8 +540,9 @@ static int launch_lb_tp(accLB_ctx* s, int c, int d, int kind, double* out_u, dou
   const int lz = s->lz;
   const dim3 grid((s->nx + LBT_TX - 1) / LBT_TX, (s->ny + LBT_TY - 1) / LBT_TY, (s->nz + lz - 1) / lz);
   LaunchScope ls(s, kind);
-  kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], s->phi[c], out_u, out_r,
-                                                        s->phi[d], s->seams, s->tabs, lz, s->tmap[c], s->tmap_row[c], in0, in1);
+  kern<<<grid, LBT_TX * LBT_TY, sizeof(T), s->stream>>>(s->kp, (const ST*)s->f[c], (ST*)s->f[d], phi_in ? phi_in : s->phi[c],
+                                                        out_u, out_r, phi_out ? phi_out : s->phi[d], s->seams, s->tabs, lz,
+                                                        s->tmap[c], s->tmap_row[c], in0, in1);
   return ACCLB_OK;
 }
 
@@ -545,6 +551,7 @@ template <int MODE>
 static int launch_lb_tp_any(accLB_ctx* s, int c, int d, int kind = KIND_LB_TP, double* out_u = nullptr,
                             double* out_r = nullptr, const double* in0 = nullptr, const double* in1 = nullptr) {
   if (MODE == MODE_UNFUSED) { out_u = s->u; out_r = s->r; }
+  if (MODE == MODE_FUSED_U) out_u = s->u;
   constexpr bool CAN_FAST = MODE != MODE_INIT;
   if (s->prm.store_fp32) {
     if (CAN_FAST && s->tmap_ok) return launch_lb_tp<float, MODE, CAN_FAST>(s, c, d, kind, out_u, out_r, in0, in1);
@@ -556,7 +563,7 @@ static int launch_lb_tp_any(accLB_ctx* s, int c, int d, int kind = KIND_LB_TP, d
 
 // The fluxes through the seam faces of the tile columns (k_seam: one launch for the three directions), after
 // k_lb_tp<FUSED> of the same step.
-static int launch_seam(accLB_ctx* s, int c, int d) {
+static int launch_seam(accLB_ctx* s, const double* phi_in, double* phi_out, bool scaled = false) {
   SeamGrid g;
   g.lz = s->lz;
   g.nchunk = (s->nz + s->lz - 1) / s->lz;
@@ -567,7 +574,8 @@ static int launch_seam(accLB_ctx* s, int c, int d) {
   g.by = blocks_for(g.nfy, SEAM_THREADS);
   g.bz = blocks_for(g.nfz, SEAM_THREADS);
   LaunchScope ls(s, KIND_SEAM);
-  k_seam<LBT_TX, LBT_TY><<<g.bx + g.by + g.bz, SEAM_THREADS, 0, s->stream>>>(s->kp, s->phi[c], s->phi[d], s->seams, g);
+  if (scaled) k_seam<LBT_TX, LBT_TY, true><<<g.bx + g.by + g.bz, SEAM_THREADS, 0, s->stream>>>(s->kp, phi_in, phi_out, s->seams, g);
+  else k_seam<LBT_TX, LBT_TY, false><<<g.bx + g.by + g.bz, SEAM_THREADS, 0, s->stream>>>(s->kp, phi_in, phi_out, s->seams, g);
   return ACCLB_OK;
 }
 
@@ -606,6 +614,19 @@ static int launch_mr_step_t(accLB_ctx* s, int c, int d) {
 }
 static int launch_mr_step(accLB_ctx* s, int c, int d) {
   return s->tmap_ok ? launch_mr_step_t<true>(s, c, d) : launch_mr_step_t<false>(s, c, d);
+}
+
+// One later stage of the SSP-RK3 integrator (R32): phi_out = a phi(t) + b (phi_in + L(phi_in; u(t))), the tiled kernel in
+// MODE_STAGE and the seam faces after it.  phi(t) = phi[c], u(t) = s->u (written by k_lb_tp<MODE_FUSED_U> of this step).
+static int launch_stage(accLB_ctx* s, int c, const double* phi_in, double* phi_out, double a, double b) {
+  s->kp.rk_a = a;
+  s->kp.rk_b = b;
+  int r = s->tmap_ok ? launch_lb_tp<double, MODE_STAGE, true>(s, c, c, KIND_STAGE, nullptr, nullptr, s->phi[c], s->u, phi_in, phi_out)
+                     : launch_lb_tp<double, MODE_STAGE, false>(s, c, c, KIND_STAGE, nullptr, nullptr, s->phi[c], s->u, phi_in, phi_out);
+  if (!r) r = launch_seam(s, phi_in, phi_out, true);
+  s->kp.rk_a = 0.0;
+  s->kp.rk_b = 1.0;
+  return r;
 }
 
 // r = D lap phi - kappa div q of a Runge-Kutta stage field (k_geom_r, phase_rk.cuh).
@@ -726,6 +747,7 @@ int accLB_create(accLB_ctx** out, int nx, int ny, int nz, const accLB_params* p,
   k.buoyant = p->gravity[0] != 0.0 || p->gravity[1] != 0.0 || p->gravity[2] != 0.0;
   k.nu = (p->tau - 0.5) / 3.0;
   k.eps_pref = k.nu / (2.0 * (1.0 / 9.0) * p->tau * p->tau);
+  k.rk_a = 0.0; k.rk_b = 1.0;
   k.zlo = p->halo_z;
   k.zhi = nz - p->halo_z;
 
@@ -793,19 +815,28 @@ int accLB_step(accLB_ctx* s, int nsteps) {
   for (int it = 0; it < nsteps; ++it) {
     const int c = s->cur, d = c ^ 1;
     if (s->prm.two_phase && s->prm.phi_integrator == 1) {
-      // SSP-RK3 for phi (R32): LB with u(t), r(phi) through HBM, then three Allen-Cahn stages with u frozen
-      int r = launch_lb_tp_any<MODE_UNFUSED>(s, c, d);
-      if (r) return r;
-      if ((r = launch_advect(s, s->phi[c], s->phi[d]))) return r;                                  // phi1 -> phi[d]
-      if ((r = launch_geom_r(s, s->phi[d]))) return r;
-      if ((r = launch_advect(s, s->phi[d], s->phis, s->phi[c], 0.75, 0.25))) return r;             // phi2 -> phis
-      if ((r = launch_geom_r(s, s->phis))) return r;
-      if ((r = launch_advect(s, s->phis, s->phi[d], s->phi[c], 1.0 / 3.0, 2.0 / 3.0))) return r;   // phi(t+1) -> phi[d]
+      // SSP-RK3 for phi (R32), u frozen at time t.  Default: the fused time step is the first stage (it also writes u(t)),
+      // the two later stages are the same tiled kernel without its LB half; each is followed by its seam faces.
+      // Variant 1: the unfused form (u, r through HBM; k_geom_r + k_advect per stage), kept for comparison.
+      int r;
+      if (s->variant == 0) {
+        if ((r = launch_lb_tp_any<MODE_FUSED_U>(s, c, d))) return r;                               // phi1 -> phi[d]
+        if ((r = launch_seam(s, s->phi[c], s->phi[d]))) return r;
+        if ((r = launch_stage(s, c, s->phi[d], s->phis, 0.75, 0.25))) return r;                    // phi2 -> phis
+        if ((r = launch_stage(s, c, s->phis, s->phi[d], 1.0 / 3.0, 2.0 / 3.0))) return r;          // phi(t+1) -> phi[d]
+      } else {
+        if ((r = launch_lb_tp_any<MODE_UNFUSED>(s, c, d))) return r;
+        if ((r = launch_advect(s, s->phi[c], s->phi[d]))) return r;                                  // phi1 -> phi[d]
+        if ((r = launch_geom_r(s, s->phi[d]))) return r;
+        if ((r = launch_advect(s, s->phi[d], s->phis, s->phi[c], 0.75, 0.25))) return r;             // phi2 -> phis
+        if ((r = launch_geom_r(s, s->phis))) return r;
+        if ((r = launch_advect(s, s->phis, s->phi[d], s->phi[c], 1.0 / 3.0, 2.0 / 3.0))) return r;   // phi(t+1) -> phi[d]
+      }
     } else if (s->prm.two_phase && s->variant == 0) {
       // default: LB + geometry + advection fused on z-marching tiles (k_lb_tp), then the seam faces (k_seam)
       int r = launch_lb_tp_any<MODE_FUSED>(s, c, d);
       if (r) return r;
-      r = launch_seam(s, c, d);
+      r = launch_seam(s, s->phi[c], s->phi[d]);
       if (r) return r;
     } else if (s->prm.two_phase) {
       // variant 1: the forward-Euler form of the unfused path, u and r through HBM (k_lb_tp<MODE_UNFUSED>, k_advect)

@@ -90,7 +90,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 //   The D3Q27 stencil weights factorise, w_i = W(cx) W(cy) W(cz) / 216 with W = (1,4,1), so every lattice stencil of
 //   PAPER.md:L104 is evaluated separably: a z combination per (x,y) column first (Sz = (1,4,1), Dz = (+1,0,-1)), then a
 //   3 x 3 stencil in the plane.  Same numbers as the 27-term sums up to rounding order.
-template <typename ST, int TX, int TY, bool FUSED>
+template <typename ST, int TX, int TY, bool FUSED, bool POP = true>
 struct GeoTile {
   // Landing zone of the pulled populations of the next plane.  For interior tiles the TMA writes population i's TX x TY box
   // of rows y0 - c_iy, plane z - c_iz, UNSHIFTED in x (TMA needs 16-byte aligned box starts, and a window widened to the next
@@ -100,7 +100,7 @@ struct GeoTile {
   // One slab per population: the box, then the TY edge elements, padded to a multiple of 128 bytes (TMA destination).
   static constexpr int TAIL_BYTES = 16 * TY <= 128 ? 128 : (16 * TY + 127) / 128 * 128;
   static constexpr int SLAB = TX * TY + TAIL_BYTES / (int)sizeof(ST);
-  alignas(128) ST fpop[Q][SLAB];
+  alignas(128) ST fpop[POP ? Q : 1][POP ? SLAB : 16];  // (no landing zone for a kernel mode that pulls no populations)
   unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
@@ -170,7 +170,10 @@ __device__ __forceinline__ double seam_face_flux(const Grid& G, const double* __
 //   MODE_DIAG     accLB_diagnostics: the sums of R21 -> rout[0..7] (warp shuffle + one atomic per block and quantity)
 //   MODE_INIT     accLB_init (R15): no pull; p* = in0, u0 = in1, A from F^s + F^p + F^b + F^g (F^nu := 0),
 //                 f_i = f_i^eq(p*, u0) - S_i(u0, A)/2 written "pushed" to x - c_i so that the first pull returns it at x
-enum { MODE_FUSED = 0, MODE_UNFUSED = 1, MODE_MOMENTS = 2, MODE_DIAG = 3, MODE_INIT = 4 };
+//   MODE_FUSED_U  MODE_FUSED that also writes u(t) -> uout: the time step + first stage of the SSP-RK3 integrator (R32)
+//   MODE_STAGE    a later Runge-Kutta stage: no populations; phi = the stage field, u(t) = in1 (frozen), base = in0 =
+//                 phi(t); phi_new = rk_a base + rk_b (phi + L(phi)) but for the seam faces (k_seam<SCALED>)       row a8
+enum { MODE_FUSED = 0, MODE_UNFUSED = 1, MODE_MOMENTS = 2, MODE_DIAG = 3, MODE_INIT = 4, MODE_STAGE = 5, MODE_FUSED_U = 6 };
 
 __device__ __forceinline__ double tp_warp_sum(double v) {
 #pragma unroll
@@ -184,11 +187,13 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         double* __restrict__ uout, double* __restrict__ rout, double* __restrict__ phi_new, Seams SM,
         const double* __restrict__ tabs, int lz, const __grid_constant__ CUtensorMap tmap_fin,
         const __grid_constant__ CUtensorMap tmap_row, const double* __restrict__ in0, const double* __restrict__ in1) {
-  constexpr bool FUSED = MODE == MODE_FUSED;
-  constexpr bool PULL = MODE != MODE_INIT;  // the populations of the current state are needed
+  constexpr bool LBF = MODE == MODE_FUSED || MODE == MODE_FUSED_U;  // the fused time step
+  constexpr bool STAGE = MODE == MODE_STAGE;
+  constexpr bool FUSED = LBF || STAGE;                              // the advection runs inside this kernel
+  constexpr bool PULL = MODE != MODE_INIT && !STAGE;  // the populations of the current state are needed
   constexpr int EC = 16 / (int)sizeof(ST);  // elements per 16-byte chunk: the edge elements of the TMA pull are fetched as aligned chunks
   static_assert(!(FAST && MODE == MODE_INIT), "the push of the initial state uses the per-thread wrap tables");
-  using T = GeoTile<ST, TX, TY, FUSED>;
+  using T = GeoTile<ST, TX, TY, FUSED, !STAGE>;
   extern __shared__ __align__(128) unsigned char smem_lb[];
   T& S = *reinterpret_cast<T*>(smem_lb);
   constexpr int NT = TX * TY;
@@ -355,6 +360,14 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   double dsum[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};  // MODE_DIAG: this thread's partial sums (7) and max |u|
   // One iteration of the march.  STEADY (FAST only): zc in [z0 + 3, z1 - 1], where every phase is active and no plane is
   // the first or the last of the chunk -- the same code with the chunk-boundary conditions resolved at compile time.
+  // MODE_STAGE: the frozen velocity of the plane updated next (loaded one iteration ahead), and the Shu-Osher combination
+  // rk_a phi(t) + rk_b (stage field + its increment) applied where a plane of phi_new is written
+  double un[3] = {0.0, 0.0, 0.0};
+  if (STAGE && active && z0 < z1) {
+    const size_t kn = (size_t)z0 * plane + o2off;
+    un[0] = __ldg(in1 + kn); un[1] = __ldg(in1 + (size_t)G.n + kn); un[2] = __ldg(in1 + 2 * (size_t)G.n + kn);
+  }
+  auto rk_out = [&](double v, size_t ko) { return STAGE ? fma(P.rk_b, v, P.rk_a * __ldg(in0 + ko)) : v; };
   auto iteration = [&](const int zc, auto steady_tag) {
     constexpr bool STEADY = decltype(steady_tag)::value;
     // ring planes zc-1+k, k = 0..3 (k = NR-1 is plane zc-2 when FUSED), as element offsets from S.raw; sb is carried
@@ -434,7 +447,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       const double php = rq[o2];
       if (adv) {
         constexpr int PX = T::PX;
-        if (FAST && tid >= NT - 2 * TY) {  // u_x of plane pz on the two x seams of the tile: 2 TY contiguous strip entries
+        if (LBF && FAST && tid >= NT - 2 * TY) {  // u_x of plane pz on the two x seams of the tile: 2 TY contiguous strip entries
           const int e = tid - (NT - 2 * TY);
           SM.sx[(((unsigned)pz * (unsigned)SM.ntx + blockIdx.x) * (unsigned)G.ny + (unsigned)y0) * 2u + (unsigned)e] =
               S.ux[(e >> 1) * TX + ((e & 1) ? TX - 1 : 0)];
@@ -455,7 +468,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
         const int cj1 = cj == 2 ? 0 : cj + 1, cj2 = cj1 == 2 ? 0 : cj1 + 1;
         double Fz = face_flux(uzm, uzc, S.col[cj][tid], S.col[cj1][tid], S.col[cj2][tid], php, ring(0)[o2], ring(1)[o2]);
         if (!STEADY) Fz = pz == z0 ? 0.0 : Fz;
-        if (STEADY || (pz > z0 && active)) __stcs(phi_new + (size_t)(pz - 1) * plane + o2off, S.acc[tid] - Fz);  // plane pz-1 is complete
+        if (STEADY || (pz > z0 && active)) {  // plane pz-1 is complete
+          const size_t ko = (size_t)(pz - 1) * plane + o2off;
+          __stcs(phi_new + ko, rk_out(S.acc[tid] - Fz, ko));
+        }
         Tp = S.e[cj][tid] - (Fx - Fxl) - Fy + Fz;
       }
       S.col[cj][tid] = php;  // plane zc-2 replaces plane zc-5
@@ -474,7 +490,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       }
       moments_of([&](int i) { return Pop<ST>::from_storage(*slot(i), i); }, M);
     }
-    if (node && !PULL) {  // MODE_INIT: p* given, no momentum, no stress (R15)
+    if (node && MODE == MODE_INIT) {  // p* given, no momentum, no stress (R15)
       M.p = __ldg(in0 + (size_t)z * plane + o2off);
       M.m[0] = M.m[1] = M.m[2] = 0.0;
 #pragma unroll
@@ -484,7 +500,10 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     if (adv) {
       Tp += ty == 0 ? 0.0 : S.fy[tid - TX];
       if (!STEADY && pz == z1 - 1) {  // the face above the chunk's last plane is a seam
-        if (active) __stcs(phi_new + (size_t)pz * plane + o2off, Tp);
+        if (active) {
+          const size_t ko = (size_t)pz * plane + o2off;
+          __stcs(phi_new + ko, rk_out(Tp, ko));
+        }
       } else {
         S.acc[tid] = Tp;
       }
@@ -527,83 +546,94 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       if (FUSED) S.e[cj][tid] -= P.kappa * divq;  // (cj was advanced above: slot of plane z = zc-1)
       else if (MODE == MODE_UNFUSED) rout[k] = P.D * lapp - P.kappa * divq;
 
-      // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
-      double Fb[3] = {0.0, 0.0, 0.0};
-      if (P.force_type != 0) {
-        const double fsz = S.ftab[0][z - z0], fcz = S.ftab[1][z - z0];
-        const double fsx = S.ftx[0][tx], fcx = S.ftx[1][tx], fsy = S.fty[0][ty], fcy = S.fty[1][ty];
-        if (P.force_type == 1) {  // ABC
-          Fb[0] = P.force_amp * (fsz + fcy);
-          Fb[1] = P.force_amp * (fsx + fcz);
-          Fb[2] = P.force_amp * (fsy + fcx);
-        } else {  // sine variant of BASELINE config 2
-          Fb[0] = P.force_amp * fsy;
-          Fb[1] = P.force_amp * fsz;
-          Fb[2] = P.force_amp * fsx;
+      if (STAGE) {  // u(t) is frozen (R32): this plane's was loaded one iteration ago, fetch the next plane's
+        S.ux[tid] = un[0];
+        S.uy[tid] = un[1];
+        uz_new = un[2];
+        if (STEADY || z + 1 < z1) {
+          const size_t kn = (size_t)k + plane;
+          un[0] = __ldg(in1 + kn); un[1] = __ldg(in1 + (size_t)G.n + kn); un[2] = __ldg(in1 + 2 * (size_t)G.n + kn);
         }
-      }
-      double A[3], rho;
-      accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, MODE != MODE_INIT, A, rho);
-      const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
-      if (FUSED) {
-        S.ux[tid] = u[0];
-        S.uy[tid] = u[1];
-        uz_new = u[2];
-        // velocities on the seams of this tile column (every strip has fewer elements than the grid has nodes: 32-bit
-        // indices).  FAST: u_x goes out one iteration later, 2 TY contiguous values from S.ux by one warp (see the
-        // advection phase); u_y only by the two warps that own the first and the last row.
-        if (!FAST) {
-          const unsigned ix = (((unsigned)z * (unsigned)SM.ntx + blockIdx.x) * (unsigned)G.ny + (unsigned)y) * 2u;
-          if (tx == 0) SM.sx[ix] = u[0];
-          if (tx == TX - 1 || x == G.nx - 1) SM.sx[ix + 1] = u[0];
+      } else {
+        // body-force density (R20): the z part of the per-axis tables is the same address for the whole block (L1 hit)
+        double Fb[3] = {0.0, 0.0, 0.0};
+        if (P.force_type != 0) {
+          const double fsz = S.ftab[0][z - z0], fcz = S.ftab[1][z - z0];
+          const double fsx = S.ftx[0][tx], fcx = S.ftx[1][tx], fsy = S.fty[0][ty], fcy = S.fty[1][ty];
+          if (P.force_type == 1) {  // ABC
+            Fb[0] = P.force_amp * (fsz + fcy);
+            Fb[1] = P.force_amp * (fsx + fcz);
+            Fb[2] = P.force_amp * (fsy + fcx);
+          } else {  // sine variant of BASELINE config 2
+            Fb[0] = P.force_amp * fsy;
+            Fb[1] = P.force_amp * fsz;
+            Fb[2] = P.force_amp * fsx;
+          }
         }
-        if (!FAST || ty == 0 || ty == TY - 1) {
-          const unsigned iy = ((unsigned)z * (unsigned)(2 * SM.nty) + 2u * blockIdx.y) * (unsigned)G.nx + (unsigned)x;
-          if (ty == 0) SM.sy[iy] = u[1];
-          if (ty == TY - 1 || y == G.ny - 1) SM.sy[iy + (unsigned)G.nx] = u[1];
+        double A[3], rho;
+        accel_from_geometry(P, M, gp, gnp, kc, phi0, Fb, MODE != MODE_INIT, A, rho);
+        const double u[3] = {M.m[0] + 0.5 * A[0], M.m[1] + 0.5 * A[1], M.m[2] + 0.5 * A[2]};  // a5, PAPER.md:L88 (R4)
+        if (LBF) {
+          S.ux[tid] = u[0];
+          S.uy[tid] = u[1];
+          uz_new = u[2];
+          // velocities on the seams of this tile column (every strip has fewer elements than the grid has nodes: 32-bit
+          // indices).  FAST: u_x goes out one iteration later, 2 TY contiguous values from S.ux by one warp (see the
+          // advection phase); u_y only by the two warps that own the first and the last row.
+          if (!FAST) {
+            const unsigned ix = (((unsigned)z * (unsigned)SM.ntx + blockIdx.x) * (unsigned)G.ny + (unsigned)y) * 2u;
+            if (tx == 0) SM.sx[ix] = u[0];
+            if (tx == TX - 1 || x == G.nx - 1) SM.sx[ix + 1] = u[0];
+          }
+          if (!FAST || ty == 0 || ty == TY - 1) {
+            const unsigned iy = ((unsigned)z * (unsigned)(2 * SM.nty) + 2u * blockIdx.y) * (unsigned)G.nx + (unsigned)x;
+            if (ty == 0) SM.sy[iy] = u[1];
+            if (ty == TY - 1 || y == G.ny - 1) SM.sy[iy + (unsigned)G.nx] = u[1];
+          }
+          if (!STEADY && z == z0) SM.sz[(2u * blockIdx.z) * plane + o2off] = u[2];
+          if (!STEADY && z == z1 - 1) SM.sz[(2u * blockIdx.z + 1u) * plane + o2off] = u[2];
         }
-        if (!STEADY && z == z0) SM.sz[(2u * blockIdx.z) * plane + o2off] = u[2];
-        if (!STEADY && z == z1 - 1) SM.sz[(2u * blockIdx.z + 1u) * plane + o2off] = u[2];
-      } else if (MODE == MODE_UNFUSED || MODE == MODE_MOMENTS) {
-        if (MODE == MODE_UNFUSED || uout) {
-          uout[k] = u[0];
-          uout[(size_t)G.n + k] = u[1];
-          uout[2 * (size_t)G.n + k] = u[2];
+        if (MODE == MODE_UNFUSED || MODE == MODE_MOMENTS || MODE == MODE_FUSED_U) {
+          if (MODE != MODE_MOMENTS || uout) {
+            uout[k] = u[0];
+            uout[(size_t)G.n + k] = u[1];
+            uout[2 * (size_t)G.n + k] = u[2];
+          }
+          if (MODE == MODE_MOMENTS && rout) rout[k] = M.p;
         }
-        if (MODE == MODE_MOMENTS && rout) rout[k] = M.p;
-      }
-      if (MODE == MODE_FUSED || MODE == MODE_UNFUSED) collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
-      if (MODE == MODE_DIAG && z >= P.zlo && z < P.zhi) {  // R21: rho |u|^2 / 2, nu a:a / (2 cs4 tau^2), phi, p*, m, max |u|;
-                                                            // a z-slab sums its own planes only
-        double a6[6];
-        hermite_coeff(M, u, A, a6);
-        const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
-        const double aa = a6[0] * a6[0] + a6[1] * a6[1] + a6[2] * a6[2] + 2.0 * (a6[3] * a6[3] + a6[4] * a6[4] + a6[5] * a6[5]);
-        dsum[0] += 0.5 * rho * uu;
-        dsum[1] += P.eps_pref * aa;
-        dsum[2] += phi0;
-        dsum[3] += M.p;
-        dsum[4] += M.m[0];
-        dsum[5] += M.m[1];
-        dsum[6] += M.m[2];
-        dsum[7] = fmax(dsum[7], sqrt(uu));
-      }
-      if (MODE == MODE_INIT) {  // R15: f_i = f_i^eq(p*, u0) - S_i(u0, A)/2, pushed to x - c_i
-        const double u0[3] = {__ldg(in1 + k), __ldg(in1 + (size_t)G.n + k), __ldg(in1 + 2 * (size_t)G.n + k)};
-        const double U[3] = {u0[0] - 0.5 * A[0], u0[1] - 0.5 * A[1], u0[2] - 0.5 * A[2]};
-        double Tt[6];
-        Tt[0] = u0[0] * u0[0] - u0[0] * A[0];
-        Tt[1] = u0[1] * u0[1] - u0[1] * A[1];
-        Tt[2] = u0[2] * u0[2] - u0[2] * A[2];
-        Tt[3] = u0[0] * u0[1] - 0.5 * (u0[0] * A[1] + u0[1] * A[0]);
-        Tt[4] = u0[0] * u0[2] - 0.5 * (u0[0] * A[2] + u0[2] * A[0]);
-        Tt[5] = u0[1] * u0[2] - 0.5 * (u0[1] * A[2] + u0[2] * A[1]);
-        double f[Q];
-        hermite2_populations(M.p, U, Tt, f);
-        ST* slab[3] = {pop_slab(fout, G, wrap_dec(z, G.nz)), pop_slab(fout, G, z), pop_slab(fout, G, wrap_inc(z, G.nz))};
-#pragma unroll
-        for (int i = 0; i < Q; ++i)
-          Pop<ST>::store(slab[1 - cz_of(i)] + ((unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)]), i, f[i]);
+        if (LBF || MODE == MODE_UNFUSED) collide_store<ST>(P, M, u, A, pop_slab(fout, G, z) + o2off, plane);
+        if (MODE == MODE_DIAG && z >= P.zlo && z < P.zhi) {  // R21: rho |u|^2 / 2, nu a:a / (2 cs4 tau^2), phi, p*, m, max |u|;
+                                                              // a z-slab sums its own planes only
+          double a6[6];
+          hermite_coeff(M, u, A, a6);
+          const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+          const double aa = a6[0] * a6[0] + a6[1] * a6[1] + a6[2] * a6[2] + 2.0 * (a6[3] * a6[3] + a6[4] * a6[4] + a6[5] * a6[5]);
+          dsum[0] += 0.5 * rho * uu;
+          dsum[1] += P.eps_pref * aa;
+          dsum[2] += phi0;
+          dsum[3] += M.p;
+          dsum[4] += M.m[0];
+          dsum[5] += M.m[1];
+          dsum[6] += M.m[2];
+          dsum[7] = fmax(dsum[7], sqrt(uu));
+        }
+        if (MODE == MODE_INIT) {  // R15: f_i = f_i^eq(p*, u0) - S_i(u0, A)/2, pushed to x - c_i
+          const double u0[3] = {__ldg(in1 + k), __ldg(in1 + (size_t)G.n + k), __ldg(in1 + 2 * (size_t)G.n + k)};
+          const double U[3] = {u0[0] - 0.5 * A[0], u0[1] - 0.5 * A[1], u0[2] - 0.5 * A[2]};
+          double Tt[6];
+          Tt[0] = u0[0] * u0[0] - u0[0] * A[0];
+          Tt[1] = u0[1] * u0[1] - u0[1] * A[1];
+          Tt[2] = u0[2] * u0[2] - u0[2] * A[2];
+          Tt[3] = u0[0] * u0[1] - 0.5 * (u0[0] * A[1] + u0[1] * A[0]);
+          Tt[4] = u0[0] * u0[2] - 0.5 * (u0[0] * A[2] + u0[2] * A[0]);
+          Tt[5] = u0[1] * u0[2] - 0.5 * (u0[1] * A[2] + u0[2] * A[1]);
+          double f[Q];
+          hermite2_populations(M.p, U, Tt, f);
+          ST* slab[3] = {pop_slab(fout, G, wrap_dec(z, G.nz)), pop_slab(fout, G, z), pop_slab(fout, G, wrap_inc(z, G.nz))};
+  #pragma unroll
+          for (int i = 0; i < Q; ++i)
+            Pop<ST>::store(slab[1 - cz_of(i)] + ((unsigned)i * plane + yrow[1 - cy_of(i)] + (unsigned)xs[1 - cx_of(i)]), i, f[i]);
+        }
       }
     }
     Pn = fma(4.0, an2, Qn); Qn = an2 - bn2;
@@ -653,12 +683,15 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
 // kinds overlap on every SM; lanes run along y for the x faces (the strips u_x[z][bx][y][s] are then contiguous) and
 // along x for the y and z faces.
 constexpr int SEAM_THREADS = 128;
+template <bool SCALED>
+__device__ __forceinline__ double seam_scale(const KP& P, double F) { return SCALED ? P.rk_b * F : F; }
 struct SeamGrid {
   unsigned nfx, nfy, nfz;  // seam faces per direction
   unsigned bx, by, bz;     // blocks per direction
   int lz, nchunk;
 };
-template <int TX, int TY>
+// SCALED: the fluxes enter phi_new times rk_b (a Runge-Kutta stage, k_lb_tp<MODE_STAGE>).
+template <int TX, int TY, bool SCALED>
 __global__ void __launch_bounds__(SEAM_THREADS) k_seam(KP P, const double* __restrict__ phi, double* __restrict__ phi_new,
                                                        Seams SM, SeamGrid SG) {
   const Grid& G = P.G;
@@ -681,7 +714,7 @@ __global__ void __launch_bounds__(SEAM_THREADS) k_seam(KP P, const double* __res
     const unsigned r = t / (unsigned)G.ny;
     const int b = (int)(r % (unsigned)SM.ntx), z = (int)(r / (unsigned)SM.ntx);
     const int c0 = b * TX, bp = b == 0 ? SM.ntx - 1 : b - 1;
-    const double F = seam_face_flux<0>(G, phi, SM, 0, y, z, c0, b, bp);
+    const double F = seam_scale<SCALED>(P, seam_face_flux<0>(G, phi, SM, 0, y, z, c0, b, bp));
     double* row = phi_new + (size_t)z * plane + (size_t)y * G.nx;
     atomicAdd(row + c0, F);
     atomicAdd(row + (c0 == 0 ? G.nx - 1 : c0 - 1), -F);
@@ -691,7 +724,7 @@ __global__ void __launch_bounds__(SEAM_THREADS) k_seam(KP P, const double* __res
     const unsigned r = t / (unsigned)G.nx;
     const int b = (int)(r % (unsigned)SM.nty), z = (int)(r / (unsigned)SM.nty);
     const int c0 = b * TY, bp = b == 0 ? SM.nty - 1 : b - 1;
-    const double F = seam_face_flux<1>(G, phi, SM, x, 0, z, c0, b, bp);
+    const double F = seam_scale<SCALED>(P, seam_face_flux<1>(G, phi, SM, x, 0, z, c0, b, bp));
     double* col = phi_new + (size_t)z * plane + x;
     atomicAdd(col + (size_t)c0 * G.nx, F);
     atomicAdd(col + (size_t)(c0 == 0 ? G.ny - 1 : c0 - 1) * G.nx, -F);
@@ -701,7 +734,7 @@ __global__ void __launch_bounds__(SEAM_THREADS) k_seam(KP P, const double* __res
     const unsigned r = t / (unsigned)G.nx;
     const int y = (int)(r % (unsigned)G.ny), b = (int)(r / (unsigned)G.ny);
     const int c0 = b * SG.lz, bp = b == 0 ? SG.nchunk - 1 : b - 1;
-    const double F = seam_face_flux<2>(G, phi, SM, x, y, 0, c0, b, bp);
+    const double F = seam_scale<SCALED>(P, seam_face_flux<2>(G, phi, SM, x, y, 0, c0, b, bp));
     double* cell = phi_new + (size_t)y * G.nx + x;
     atomicAdd(cell + (size_t)c0 * plane, F);
     atomicAdd(cell + (size_t)(c0 == 0 ? G.nz - 1 : c0 - 1) * plane, -F);

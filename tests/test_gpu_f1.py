@@ -16,12 +16,13 @@ def both(acclb, cfg, shape=None, **extra):
     return gpu_sim(acclb, cfg, shape=shape, **extra), cpu_sim(cfg, shape=shape)
 
 
-@pytest.mark.parametrize("rk3", [0, 1])
+@pytest.mark.parametrize("rk3,variant", [(0, 0), (1, 0), (1, 1)])
 @pytest.mark.parametrize("shape", [(64, 32, 24), (40, 26, 22)])
-def test_buoyant_two_phase_density_ratio_100(acclb, shape, rk3):
+def test_buoyant_two_phase_density_ratio_100(acclb, shape, rk3, variant):
     """Density contrast 100, nu = 0.005 (tau = 0.515), zero gauge pressure, gravity along -z with the mean density as
     reference, ABC forcing, a droplet straddling the periodic corner: tile-divisible (TMA path) and ragged boxes, forward
-    Euler and SSP-RK3.  F^p, F^nu, F^g and A = F / rho all carry weight here."""
+    Euler and SSP-RK3 (variant 0: the stages run in the tiled kernel, the first one fused with the LB step; variant 1:
+    u and r through HBM, k_geom_r + k_advect per stage).  F^p, F^nu, F^g and A = F / rho all carry weight here."""
     rho, u, phi = ragged_two_phase(shape, 100.0)
     dens = 1.0 + 99.0 * phi
     cfg = dict(n=None, rho=rho, u=0.2 * u, phi=phi,
@@ -29,6 +30,7 @@ def test_buoyant_two_phase_density_ratio_100(acclb, shape, rk3):
                            force_type=1, force_amp=1e-6, force_k=1, gravity=(0.0, 1e-7, -2e-6), rho_ref=float(dens.mean()),
                            phi_rk3=rk3))
     sim, o = both(acclb, cfg, shape=shape)
+    sim.set_variant(variant)
     assert_parity(sim, o, what="t=0")
     for t in (1, 9, 10):
         sim.step(t)
