@@ -400,6 +400,21 @@ def run_cuda(args):
                 "of_population_roofline": g * lb_bytes_per_lup(False) / hbm_peak()[0],
                 "of_own_roofline": g * lb_bytes_per_lup(False, True) / hbm_peak()[0],
                 "note": "SM-latency-bound (two barriers per plane, 16 warps per SM), not HBM-bound"}
+        if not args.fp32 and not args.rk3:
+            # SURVEY 8(f) #1 and #3 on the same inputs: the SSP-RK3 integrator of phi, and the step as one z-slab with its halo
+            # exchange (this GPU as its own neighbour)
+            rk_cfg = dict(cfg, params=dict(cfg["params"], phi_rk3=1))
+            rk = measure_cuda(rk_cfg, args.steps, args.warmup, local_rank=local_rank, e2e=False)
+            line["two_phase_rk3"] = {"workload": f"{args.workload} {args.n}^3 two-phase, SSP-RK3 integrator of phi (three stages per step)",
+                                     "value": n3 * args.steps / (rk["ms"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": rk["ms"] / args.steps,
+                                     "gpu_launches": rk["launches"], "clocks": rk["clocks"],
+                                     "kernels_ms_per_step": {k: v[0] / args.steps for k, v in rk["kernels"].items() if v[1]}}
+            sl = measure_slab(cfg, args.n, args.steps, args.warmup, local_rank=local_rank)
+            line["z_slab"] = {"workload": f"{args.workload} {args.n}^3 two-phase as ONE z-slab of {args.n} own planes + {sl['halo']} halo planes "
+                                          "per side, halo exchange after every step (the rank is its own neighbour: device copies)",
+                              "value": n3 * args.steps / (sl["ms"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": sl["ms"] / args.steps,
+                              "exchange_ms_per_step": sl["exchange_ms"] / args.steps, "halo_bytes_sent_per_step": sl["halo_bytes"],
+                              "gpu_launches": sl["launches"], "clocks": sl["clocks"]}
         line["single_phase"] = {"workload": f"hit {args.n}^3 single-phase; " + WORKLOADS["hit"][1],
                                 "value": n3 * args.steps / (sp["ms"] * 1e-3) / 1e9, "unit": UNIT,
                                 "ms_per_step": sp["ms"] / args.steps, "gpu_launches": sp["launches"], "clocks": sp["clocks"],
@@ -418,61 +433,79 @@ def run_cuda(args):
 
 
 # ------------------------------------------------------------------------------------------------------ z-slabs (8(f) #3)
-def run_slabs(args):
-    """`--slabs`: ONE periodic domain n x n x (n * N) cut into N z-slabs, one per rank / GPU (the shape of the paper's weak
-    scaling, PAPER.md:L126), halo exchange after every step inside the timed region (NCCL send / recv between the ranks;
-    with N = 1 the rank is its own neighbour and the exchange is device copies).  The fields are the n^3 workload repeated
-    along z.  Not the driver's line: `python bench.py --gpus N` without --slabs stays "replicas only"."""
+def measure_slab(cfg, n, steps, warmup, *, rank=0, world=1, local_rank=0, fp32=False, barrier=None):
+    """Time `steps` steps of this rank's z-slab (n own planes + halos) of an n x n x (n * world) domain, the halo exchange
+    after every step inside the timed region.  The n^3 fields of `cfg` repeat along z."""
     import numpy as np
     import torch
 
-    from paper_2505_01126_b200 import build as _build, slabs
+    from paper_2505_01126_b200 import slabs
 
-    rank, local_rank, world = dist_env()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the CUDA arm has no CPU fallback)")
-    torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    barrier = lambda: None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl", device_id=dev)
-        barrier = dist.barrier
-    if rank == 0:
-        _build.build()
-    barrier()
-    n = args.n
-    cfg = make_workload(args.workload, n)
-    two_phase = bool(cfg["params"]["two_phase"])
-    part = slabs.SlabAccLB(n, n, n * world, rank=rank, world=world, device=local_rank, store_fp32=int(args.fp32), **cfg["params"])
+    sync = barrier or (lambda: None)
+    part = slabs.SlabAccLB(n, n, n * world, rank=rank, world=world, device=local_rank, store_fp32=int(fp32), **cfg["params"])
     sl = part.slab
-    planes = np.arange(sl.z_origin, sl.z_origin + sl.nz_local) % n   # the n^3 fields repeat along z
+    planes = np.arange(sl.z_origin, sl.z_origin + sl.nz_local) % n
     loc = {k: torch.from_numpy(np.ascontiguousarray(np.take(cfg[k], planes, axis=1 if k == "u" else 0))).to(dev)
            for k in ("rho", "u", "phi") if cfg[k] is not None}
     part.init(loc["rho"], loc["u"], loc.get("phi"))
-    part.step(args.warmup)
+    part.step(warmup)
     torch.cuda.synchronize(dev)
     d0 = part.diagnostics()
     stream = torch.cuda.current_stream(dev)
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps + 1)]
     launches0 = part.sim.launch_count
-    barrier()
+    sync()
     torch.cuda.synchronize(dev)
     with ClockSampler(local_rank) as clk:
         ev[0].record(stream)
-        for t in range(args.steps):
+        for t in range(steps):
             part.sim.step(1)
             ev[2 * t + 1].record(stream)
             part.exchange()
             ev[2 * t + 2].record(stream)
         torch.cuda.synchronize(dev)
-    barrier()
-    launches = part.sim.launch_count - launches0  # the copies / NCCL kernels of the exchange are not counted
-    ms = ev[0].elapsed_time(ev[-1])
-    ms_x = sum(ev[2 * t + 1].elapsed_time(ev[2 * t + 2]) for t in range(args.steps))
-    d1 = part.diagnostics()
-    ms, ms_x = max_over_ranks([ms, ms_x], f"cuda:{local_rank}" if world > 1 else None)
+    sync()
+    out = {"ms": ev[0].elapsed_time(ev[-1]),
+           "exchange_ms": sum(ev[2 * t + 1].elapsed_time(ev[2 * t + 2]) for t in range(steps)),
+           "launches": part.sim.launch_count - launches0,  # the copies / NCCL kernels of the exchange are not counted
+           "clocks": clk.summary(), "halo_bytes": part.halo_bytes_per_step(), "halo": sl.halo, "nz_local": sl.nz_local,
+           "diag0": d0, "diag1": part.diagnostics()}
+    part.close()
+    del loc
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_slabs(args):
+    """`--slabs`: ONE periodic domain n x n x (n * N) cut into N z-slabs, one per rank / GPU (the shape of the paper's weak
+    scaling, PAPER.md:L126), halo exchange after every step inside the timed region (NCCL send / recv between the ranks;
+    with N = 1 the rank is its own neighbour and the exchange is device copies).  The fields are the n^3 workload repeated
+    along z.  Not the driver's line: `python bench.py --gpus N` without --slabs stays "replicas only"."""
+    import torch
+
+    from paper_2505_01126_b200 import build as _build
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA arm has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    barrier = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        barrier = dist.barrier
+    if rank == 0:
+        _build.build()
+    if barrier:
+        barrier()
+    n = args.n
+    cfg = make_workload(args.workload, n)
+    two_phase = bool(cfg["params"]["two_phase"])
+    m = measure_slab(cfg, n, args.steps, args.warmup, rank=rank, world=world, local_rank=local_rank, fp32=bool(args.fp32),
+                     barrier=barrier)
+    ms, ms_x = max_over_ranks([m["ms"], m["exchange_ms"]], f"cuda:{local_rank}" if world > 1 else None)
     if rank == 0:
         own = n ** 3
         bpl = step_bytes_per_lup(bool(args.fp32), two_phase)
@@ -483,18 +516,16 @@ def run_slabs(args):
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": f"{args.workload} {n} x {n} x {n * world} {'two' if two_phase else 'single'}-phase, one periodic "
-                                   f"domain in {world} z-slab(s) of {n} planes + {sl.halo} halo planes per side; the {n}^3 fields "
+                                   f"domain in {world} z-slab(s) of {n} planes + {m['halo']} halo planes per side; the {n}^3 fields "
                                    "repeated along z; " + WORKLOADS[args.workload][1],
                        "parallelism": f"z-slabs x{world}, one halo exchange per step ("
                                       + ("NCCL send/recv" if world > 1 else "the rank is its own neighbour: device copies") + ")",
-                       "halo_bytes_sent_per_rank_and_step": part.halo_bytes_per_step(),
-                       "lups_per_step": world * own, "planes_computed_per_rank": sl.nz_local},
-            "exchange_ms_per_step": ms_x / args.steps, "clocks": clk.summary(),
-            "gpu_launches": launches,
+                       "halo_bytes_sent_per_rank_and_step": m["halo_bytes"],
+                       "lups_per_step": world * own, "planes_computed_per_rank": m["nz_local"]},
+            "exchange_ms_per_step": ms_x / args.steps, "clocks": m["clocks"], "gpu_launches": m["launches"],
             "roofline": {"bound": "hbm", "scope": "whole step incl. halo exchange, own planes only", "unit": "GB/s", "peak": peak * world,
                          "peak_source": how, "achieved": value * bpl, "frac": value * bpl / (peak * world), "traffic": None},
-            "diagnostics": {"before": d0, "after": d1}}), flush=True)
-    part.close()
+            "diagnostics": {"before": m["diag0"], "after": m["diag1"]}}), flush=True)
     if world > 1:
         torch.distributed.destroy_process_group()
 
@@ -539,7 +570,8 @@ def main():
     ap.add_argument("--moment-storage", type=int, default=0, help="1: single-phase state = the ten fields (p*, u, a) per node (SURVEY 8(f) #2); use with --workload hit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--no-single", action="store_true", help="skip the single_phase leg of a two-phase run")
+    ap.add_argument("--no-single", action="store_true", help="skip the extra legs of a two-phase run (single_phase, "
+                                                             "single_phase_moment_storage, two_phase_rk3, z_slab)")
     ap.add_argument("--slabs", action="store_true", help="one domain n x n x (n N) in N z-slabs with halo exchange (SURVEY 8(f) #3) "
                                                          "instead of N independent replicas")
     ap.add_argument("--sweep", action="store_true")
