@@ -107,11 +107,13 @@ __device__ __forceinline__ double weno5_minus_c(double d1, double d2, double d3,
   const double r2 = __fma_rn(13.0, __dmul_rn(s2, s2), __fma_rn(3.0, __dmul_rn(t2, t2), eps12));
   const double e0 = __dmul_rn(r0, r0), e1 = __dmul_rn(r1, r1), e2 = __dmul_rn(r2, r2);
   const double m0 = __dmul_rn(e1, e2), m1 = __dmul_rn(e0, e2), m2 = __dmul_rn(e0, e1);  // weights d_k m_k, d = (.1,.6,.3)
-  const double x0 = __fma_rn(0.5, d2, __dmul_rn(-0.2, d1));  // 0.1 * 6 (q0 - c)
-  const double x1 = __fma_rn(1.2, d3, __dmul_rn(0.6, d2));   // 0.6 * 6 (q1 - c)
-  const double x2 = __fma_rn(1.2, d3, __dmul_rn(-0.3, d4));  // 0.3 * 6 (q2 - c)
+  // numerator and denominator both times 5: every constant is then a multiple of 1/2, which the fp64 instructions take as
+  // an immediate operand (0.2, 0.6, 1.2 ... need two uniform-register moves each, at every use)
+  const double x0 = __fma_rn(2.5, d2, -d1);                   // 5 * 0.1 * 6 (q0 - c)
+  const double x1 = __fma_rn(6.0, d3, __dmul_rn(3.0, d2));    // 5 * 0.6 * 6 (q1 - c)
+  const double x2 = __fma_rn(6.0, d3, __dmul_rn(-1.5, d4));   // 5 * 0.3 * 6 (q2 - c)
   const double num = __fma_rn(m2, x2, __fma_rn(m1, x1, __dmul_rn(m0, x0)));
-  const double den = __fma_rn(1.8, m2, __fma_rn(3.6, m1, __dmul_rn(0.6, m0)));  // 6 (0.1 m0 + 0.6 m1 + 0.3 m2)
+  const double den = __fma_rn(9.0, m2, __fma_rn(18.0, m1, __dmul_rn(3.0, m0)));  // 5 * 6 (0.1 m0 + 0.6 m1 + 0.3 m2)
   return div_pos(num, den);
 }
 
