@@ -198,6 +198,20 @@ int accLB_stats_pdf(const double* u, int nx, int ny, int nz, int r, double scale
 int accLB_stats_spectrum(const double* uhat, int nx, int ny, int nz, int ncomp, int nshell, double* E, void* scratch,
                          size_t scratch_bytes, int device, void* stream);
 
+/* ---- The same structure functions for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): accLB_stats_increments without the caller's scratch block.  The
+ * accumulators (3 nr doubles) live in ONE fixed array of device memory inside the library (file scope, 256-byte aligned,
+ * 3 * ACCLB_STATS_STATIC_MAX_NR doubles = 1536 bytes; every GPU that loads the library holds it until the process exits).
+ * The call allocates nothing: no cudaMalloc / cudaFree, no allocating library routine; it zeroes the accumulators it uses,
+ * launches the same kernel as accLB_stats_increments, copies the 3 nr sums to `out` (HOST) and synchronises `stream`.
+ *   u, r, nr, out, device, stream: as for accLB_stats_increments.  nr > ACCLB_STATS_STATIC_MAX_NR -> ACCLB_EINVAL.
+ * ALL calls on a device share the array, which keeps the last call's contents: two calls that overlap on the GPU (different
+ * streams, or different host threads) race on it and give wrong sums -- serialise them, or use accLB_stats_increments with
+ * one scratch block per caller. */
+#define ACCLB_STATS_STATIC_MAX_NR 64
+int accLB_stats_increments_static(const double* u, int nx, int ny, int nz, const int* r, int nr, double* out, int device,
+                                  void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,8 @@ ERRORS = {0: "ACCLB_OK", -1: "ACCLB_EINVAL", -2: "ACCLB_EWORKSPACE", -3: "ACCLB_
 SYMBOLS = ("accLB_workspace_bytes", "accLB_create", "accLB_init", "accLB_step", "accLB_moments",
            "accLB_diagnostics", "accLB_run_host", "accLB_launch_count", "accLB_profile",
            "accLB_profile_read", "accLB_set_variant", "accLB_halo_chunks", "accLB_destroy",
-           "accLB_last_error", "accLB_stats_increments", "accLB_stats_pdf", "accLB_stats_spectrum")
+           "accLB_last_error", "accLB_stats_increments", "accLB_stats_pdf", "accLB_stats_spectrum",
+           "accLB_stats_increments_static")
 
 
 class Params(C.Structure):
@@ -91,6 +92,8 @@ def load():
                                   C.POINTER(C.c_ulonglong), _dp, C.c_size_t, C.c_int, C.c_void_p]
     L.accLB_stats_spectrum.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), _dp, C.c_size_t,
                                        C.c_int, C.c_void_p]
+    L.accLB_stats_increments_static.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_double),
+                                                C.c_int, C.c_void_p]
     _lib = L
     return L
 
@@ -256,6 +259,22 @@ def stats_increments(u, separations):
     scratch = torch.empty(3 * nr, dtype=torch.float64, device=dev)
     _check(load().accLB_stats_increments(u.data_ptr(), nx, ny, nz, r, nr, out, scratch.data_ptr(), scratch.numel() * 8,
                                          dev.index or 0, stream))
+    return [[out[3 * j + p] for p in range(3)] for j in range(nr)]
+
+
+STATS_STATIC_MAX_NR = 64
+
+
+def stats_increments_static(u, separations):
+    """stats_increments through the entry point that allocates nothing: the accumulators are a fixed array inside the library
+    (at most STATS_STATIC_MAX_NR separations; calls on one device share it and must not overlap).  Array [nr][3]."""
+    torch, dev, stream = _stats_common(u, 4)
+    assert u.dtype == torch.float64 and u.shape[0] == 3
+    _, nz, ny, nx = u.shape
+    nr = len(separations)
+    r = (C.c_int * nr)(*[int(v) for v in separations])
+    out = (C.c_double * (3 * nr))()
+    _check(load().accLB_stats_increments_static(u.data_ptr(), nx, ny, nz, r, nr, out, dev.index or 0, stream))
     return [[out[3 * j + p] for p in range(3)] for j in range(nr)]
 
 

@@ -21,6 +21,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1131,6 +1132,57 @@ int accLB_stats_spectrum(const double* uhat, int nx, int ny, int nz, int ncomp, 
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(E, acc, (size_t)nshell * sizeof(double), cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
+  return ACCLB_OK;
+}
+
+// ---------------------------------------------------------------------------------------- no-allocation entry point
+// Accumulators of accLB_stats_increments_static: device memory that belongs to the library image (one copy per GPU that loads
+// it).  In host code `g_stats_static` is only a handle for the runtime, not a device address: the address a kernel can use
+// comes from cudaGetSymbolAddress, asked for once per device with that device current.
+static __device__ __align__(256) double g_stats_static[3 * ACCLB_STATS_STATIC_MAX_NR];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+static double* g_stats_static_ptr[STATIC_MAX_DEVICES];  // per device; nullptr = not asked for yet
+static std::mutex g_stats_static_mutex;
+
+// Device address of g_stats_static on `device`, which must be the current device.
+static int stats_static_address(int device, double** ptr) {
+  if (device < 0 || device >= STATIC_MAX_DEVICES) return fail(ACCLB_EINVAL, "accLB_stats_increments_static: device %d", device);
+  std::lock_guard<std::mutex> lock(g_stats_static_mutex);
+  if (!g_stats_static_ptr[device]) {
+    double* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&p, g_stats_static);
+    if (e != cudaSuccess || !p)
+      return fail(ACCLB_ECUDA, "accLB_stats_increments_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+    g_stats_static_ptr[device] = p;
+  }
+  *ptr = g_stats_static_ptr[device];
+  return ACCLB_OK;
+}
+
+int accLB_stats_increments_static(const double* u, int nx, int ny, int nz, const int* r, int nr, double* out, int device,
+                                  void* stream) {
+  if (!u || !r || !out || nr < 1 || nx < 1 || ny < 1 || nz < 1 || (double)nx * ny * nz >= 2147483648.0)
+    return fail(ACCLB_EINVAL, "accLB_stats_increments_static: bad argument");
+  if (nr > ACCLB_STATS_STATIC_MAX_NR)
+    return fail(ACCLB_EINVAL, "accLB_stats_increments_static: nr = %d separations, the built-in scratch holds at most %d "
+                              "(use accLB_stats_increments with a scratch block of your own)", nr, ACCLB_STATS_STATIC_MAX_NR);
+  for (int j = 0; j < nr; ++j)
+    if (r[j] < 0) return fail(ACCLB_EINVAL, "accLB_stats_increments_static: negative separation");
+  DeviceGuard guard_(device);
+  if (!guard_.ok) return fail(ACCLB_ECUDA, "accLB_stats_increments_static: cannot select device %d", device);
+  double* acc = nullptr;
+  int rc = stats_static_address(device, &acc);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Grid G{nx, ny, nz, (unsigned)((size_t)nx * ny * nz)};
+  CK(cudaMemsetAsync(acc, 0, (size_t)nr * 3 * sizeof(double), st));  // the array keeps the last call's sums
+  for (int j = 0; j < nr; ++j) k_stats_increments<<<stats_blocks(G.n), STATS_THREADS, 0, st>>>(G, u, r[j], acc + 3 * j);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, acc, (size_t)nr * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  const double inv = 1.0 / (3.0 * (double)G.n);
+  for (int j = 0; j < 3 * nr; ++j) out[j] *= inv;
   return ACCLB_OK;
 }
 
