@@ -332,19 +332,21 @@ def test_p12_axis_permutation_and_reflection():
 
 
 # ------------------------------------------------------------------ sub-box evaluation used by the full-size GPU parity test
-def test_subbox_evaluation_matches_full_box_interior():
-    """k steps only depend on inputs within radius 3k (two-phase) of a node: running the oracle on a periodic
-    sub-box reproduces the full-box values away from the sub-box rim."""
-    n, s, k = 24, 18, 2
+@pytest.mark.parametrize("rk3,n,s,k", [(0, 24, 18, 2), (1, 32, 28, 1)])
+def test_subbox_evaluation_matches_full_box_interior(rk3, n, s, k):
+    """k steps only depend on inputs within radius 3k (two-phase, forward Euler) of a node, 9k with the three-stage
+    Runge-Kutta integrator of phi (each stage reaches 3 further, R32): running the oracle on a periodic sub-box reproduces
+    the full-box values away from the sub-box rim."""
     cfg = wl.make_config("bubbly", n=n)
+    cfg["params"]["phi_rk3"] = rk3
     cfg["phi"] = wl.bubbles_phi(n, np.array([[9.0, 10.0, 11.0]]), radius=5.0)
     full = run(cfg, k).moments()
-    org = (20, 3, 15)                                   # wraps across the periodic boundary in x
+    org = (n - 4, 3, n - 9)                             # wraps across the periodic boundary in x
     sub = oracle.Oracle(s, s, s, **cfg["params"], force_period=(n, n, n), force_origin=org)
     sub.init(wl.subbox(cfg["rho"], org, s), wl.subbox(cfg["u"], org, s), wl.subbox(cfg["phi"], org, s))
     sub.step(k)
     got = sub.moments()
-    rim = 3 * k + 2
+    rim = (9 if rk3 else 3) * k + 2
     inner = (slice(rim, s - rim),) * 3
     for a, b in zip(full, got):
         assert np.abs(wl.subbox(a, org, s)[..., inner[0], inner[1], inner[2]] - b[..., inner[0], inner[1], inner[2]]).max() < 1e-15
