@@ -665,10 +665,11 @@ static int make_tensor_maps(accLB_ctx* s) {
   if (s->nx % LBT_TX != 0 || s->ny % LBT_TY != 0) return 0;  // FAST: every tile full
   const cuuint64_t dims[3] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny, (cuuint64_t)(s->prm.moment_storage ? 10 : 27) * s->nz};
   const cuuint64_t strides[2] = {(cuuint64_t)s->nx * es, (cuuint64_t)s->nx * s->ny * es};
-  const cuuint32_t box[3] = {LBT_TX, LBT_TY, 1}, row[3] = {LBT_TX, 1, 1}, estr[3] = {1, 1, 1};
+  // two-phase: one box fetches the three populations of a triple (twophase.cuh); moment storage: one field per box
+  const cuuint32_t box[3] = {LBT_TX, LBT_TY, s->prm.moment_storage ? 1u : 3u}, row[3] = {LBT_TX, 1, 1}, estr[3] = {1, 1, 1};
   for (int b = 0; b < 2; ++b) {
     CUresult r = ((encode_t)fn)(&s->tmap[b], dt, 3, s->f[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,  // (128 B / 256 B promotion measured: no difference)
                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return 0;
     r = ((encode_t)fn)(&s->tmap_row[b], dt, 3, s->f[b], dims, strides, row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,

@@ -96,11 +96,15 @@ struct GeoTile {
   // of rows y0 - c_iy, plane z - c_iz, UNSHIFTED in x (TMA needs 16-byte aligned box starts, and a window widened to the next
   // aligned element costs a 64-byte DRAM fetch per row: measured +4.8 GB per 512^3 step), so thread tx reads element
   // tx - c_ix of its row; the one element per row that lies outside the box (x0 - 1 for c_ix = +1, x0 + TX for c_ix = -1)
-  // is fetched by the edge lane itself with an 8-byte cp.async into the tail of the slab.
-  // One slab per population: the box, then the TY edge elements, padded to a multiple of 128 bytes (TMA destination).
-  static constexpr int TAIL_BYTES = 16 * TY <= 128 ? 128 : (16 * TY + 127) / 128 * 128;
-  static constexpr int SLAB = TX * TY + TAIL_BYTES / (int)sizeof(ST);
-  alignas(128) ST fpop[POP ? Q : 1][POP ? SLAB : 16];  // (no landing zone for a kernel mode that pulls no populations)
+  // is fetched by lanes of the row's warp as aligned 16-byte chunks (cp.async) into the tail of the slab.
+  // The three populations i = 3 m, 3 m + 1, 3 m + 2 (c_ix = -1, 0, +1; same c_iy, c_iz) are consecutive planes of the
+  // [z][i][y][x] layout with the same box origin: ONE TMA box TX x TY x 3 fetches them (9 instead of 27 issues per plane).
+  // One slab per triple: the three boxes back to back, then the TY edge chunks of population 3 m, then those of 3 m + 2.
+  static constexpr int TAILE = 16 / (int)sizeof(ST) * TY;   // elements of one population's edge chunks
+  static constexpr int TRIPLE = 3 * TX * TY + 2 * TAILE;
+  static_assert(!POP || (TRIPLE * sizeof(ST)) % 128 == 0, "TMA destinations are 128-byte aligned");
+  __host__ __device__ static constexpr int pop_off(int i) { return (i / 3) * TRIPLE + (i % 3) * (TX * TY); }  // box of population i in fpop
+  alignas(128) ST fpop[POP ? (Q / 3) * TRIPLE : 16];  // (no landing zone for a kernel mode that pulls no populations)
   unsigned long long fbar;  // mbarrier of the TMA pull
   static constexpr int PX = TX + 4, PY = TY + 4;  // phi planes: tile + halo 2
   static constexpr int NX = TX + 2, NY = TY + 2;  // n, q planes: tile + halo 1
@@ -252,25 +256,34 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
     yrow[2] = (unsigned)wrap_inc(yw, G.ny) * (unsigned)G.nx;
   }
   // three per-thread bases, one per c_ix, so that slot(i) is base + a compile-time offset
-  ST* const sl_c = &S.fpop[0][ty * TX + tx];
-  // (FAST: the slab's tail holds, per tile row, the aligned 16-byte chunk that ends at x0-1 (c_ix = +1) / starts at x0+TX (-1))
-  ST* const sl_p = tx == 0 ? &S.fpop[0][NT + (fast ? EC * ty + EC - 1 : ty)] : sl_c - 1;  // c_ix = +1: element x - 1
-  ST* const sl_m = tx == TX - 1 ? &S.fpop[0][NT + (fast ? EC * ty : ty)] : sl_c + 1;       // c_ix = -1: element x + 1
-  auto slot = [&](int i) -> ST* { return (cx_of(i) == 0 ? sl_c : cx_of(i) == 1 ? sl_p : sl_m) + i * T::SLAB; };
-  // The TMA issue is spread over the block's warps (warp w issues boxes w, w + TY, ...): one thread issuing all 27 made
-  // its warp arrive late at the next barrier in every iteration.  Thread 0 arms the mbarrier with the byte count.
+  ST* const sl_c = &S.fpop[ty * TX + tx];
+  // (FAST: the slab's tail holds, per tile row, the aligned 16-byte chunk that ends at x0-1 (c_ix = +1) / starts at x0+TX (-1);
+  // the edge lanes' bases are chosen so that base + pop_off(i) is the tail element: pop_off(3 m + 2) = m TRIPLE + 2 NT,
+  // pop_off(3 m) = m TRIPLE)
+  ST* const sl_p = tx == 0 ? &S.fpop[NT + T::TAILE + (fast ? EC * ty + EC - 1 : ty)] : sl_c - 1;  // c_ix = +1: element x - 1
+  ST* const sl_m = tx == TX - 1 ? &S.fpop[3 * NT + (fast ? EC * ty : ty)] : sl_c + 1;              // c_ix = -1: element x + 1
+  auto slot = [&](int i) -> ST* { return (cx_of(i) == 0 ? sl_c : cx_of(i) == 1 ? sl_p : sl_m) + T::pop_off(i); };
+  // The TMA issue is spread over the block's warps (the last warp issues triples 0 and TY, the others one each; the first
+  // warps carry the rim items of the derive pass): one thread issuing everything made its warp arrive late at the next
+  // barrier in every iteration.  Thread 0 arms the mbarrier with the byte count.
   auto tma_pull = [&](int z) {  // called by lanes 0..TY-1 of every warp, after the block-wide hand-over of the landing zone
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (tid == 0) mbar_arrive_expect_tx(&S.fbar, (unsigned)(Q * NT * sizeof(ST)));
     const int zs[3] = {wrap_dec(z, G.nz) * Q, z * Q, wrap_inc(z, G.nz) * Q};
 #pragma unroll
-    for (int k = 0; k < (Q + TY - 1) / TY; ++k) {
-      const int i = ty + k * TY;
-      if (i < Q) {
-        const int cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
-        const int slab = (cz < 0 ? zs[2] : cz > 0 ? zs[0] : zs[1]) + i;
-        if (yrim && cy != 0) tma_load_box(&S.fpop[i][tx * TX], &tmap_row, x0, pmod(y0 - cy + tx, G.ny), slab, &S.fbar);
-        else if (tx == 0) tma_load_box(&S.fpop[i][0], &tmap_fin, x0, y0 - cy, slab, &S.fbar);
+    for (int k = 0; k < (Q / 3 + TY - 1) / TY; ++k) {
+      const int m = (TY - 1 - ty) + k * TY;  // triple: populations 3 m .. 3 m + 2, c_iy = m % 3 - 1, c_iz = m / 3 - 1
+      if (m < Q / 3) {
+        const int cy = m % 3 - 1, cz = m / 3 - 1;
+        const int slab = (cz < 0 ? zs[2] : cz > 0 ? zs[0] : zs[1]) + 3 * m;
+        ST* dst = &S.fpop[m * T::TRIPLE];
+        if (yrim && cy != 0) {
+          const int yy = pmod(y0 - cy + tx, G.ny);
+#pragma unroll
+          for (int j = 0; j < 3; ++j) tma_load_box(dst + j * NT + tx * TX, &tmap_row, x0, yy, slab + j, &S.fbar);
+        } else if (tx == 0) {
+          tma_load_box(dst, &tmap_fin, x0, y0 - cy, slab, &S.fbar);
+        }
       }
     }
   };
@@ -285,7 +298,6 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   // FAST: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
   // c_ix = -1) are fetched by lanes 0..17 of the row's warp, one 16-byte cp.async each (the aligned pair that holds the
   // element), into the tail of the slabs
-  static_assert(TY * 16 <= T::TAIL_BYTES, "edge chunks fit the slab tail");
   unsigned e_off = 0;  // i * plane + row + column of this lane's edge pair
   if (fast && tx < 18) {
     const int m = tx < 9 ? tx : tx - 9;
@@ -298,7 +310,7 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
       if (tx < 18) {
         const int m = tx < 9 ? tx : tx - 9;  // population 3 m + 2 (c_ix = +1) or 3 m (c_ix = -1), c_iz = m / 3 - 1
         const ST* sl = pop_slab(fin, G, m < 3 ? wrap_inc(z, G.nz) : m >= 6 ? wrap_dec(z, G.nz) : z);
-        cp_async_16(&S.fpop[3 * m + (tx < 9 ? 2 : 0)][NT + EC * ty], sl + e_off);
+        cp_async_16(&S.fpop[m * T::TRIPLE + 3 * NT + (tx < 9 ? T::TAILE : 0) + EC * ty], sl + e_off);
       }
       cp_async_commit();
       return;
