@@ -237,8 +237,8 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   }
 
   // a1: pull-stream of plane z, f_i(x,t) = f*_i(x - c_i, t-1).
-  // FAST: 27 tiled TMA loads per plane (cp.async.bulk.tensor, issued by lane 0 of the block's warps, three or four boxes
-  // each), completion counted in bytes on an mbarrier; no per-thread copy instructions, no address registers held by
+  // FAST: 9 tiled TMA loads per plane (cp.async.bulk.tensor, one TX x TY x 3 box per triple of populations, issued by
+  // lane 0 of the block's warps), completion counted in bytes on an mbarrier; no per-thread copy instructions, no address registers held by
   // copies in flight, no L1 allocation.  Lanes 0..17 of a row fetch the 9 + 9 elements per row outside the boxes.
   // Otherwise: one 8-byte cp.async per thread and population.  Either way population i of thread (tx, ty) is at *slot(i).
   constexpr bool fast = FAST;
