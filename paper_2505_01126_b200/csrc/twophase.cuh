@@ -298,19 +298,28 @@ k_lb_tp(KP P, const ST* __restrict__ fin, ST* __restrict__ fout, const double* _
   // FAST: the 9 + 9 elements per tile row that lie outside the unshifted boxes (x0 - 1 for c_ix = +1, x0 + TX for
   // c_ix = -1) are fetched by lanes 0..17 of the row's warp, one 16-byte cp.async each (the aligned pair that holds the
   // element), into the tail of the slabs
-  unsigned e_off = 0;  // i * plane + row + column of this lane's edge pair
+  // Carried per lane: the source address of its chunk for the plane pulled next (the calls go z0, z0 + 1, ...: the address
+  // advances by one z slab per call and wraps with the lane's source plane z - c_iz), its landing address, and the z at
+  // which the source plane wraps -- instead of a 64-bit slab product and the index arithmetic in every iteration.
+  const ST* e_src = fin;
+  unsigned e_dst = 0;
+  int e_zwrap = 0;
   if (fast && tx < 18) {
-    const int m = tx < 9 ? tx : tx - 9;
-    const int e_i = 3 * m + (tx < 9 ? 2 : 0), cy = m % 3 - 1;
-    e_off = (unsigned)e_i * plane + (unsigned)pmod(y - cy, G.ny) * (unsigned)G.nx +
-            (unsigned)(tx < 9 ? pmod(x0 - EC, G.nx) : pmod(x0 + TX, G.nx));
+    const int m = tx < 9 ? tx : tx - 9;  // population 3 m + 2 (c_ix = +1) or 3 m (c_ix = -1), c_iz = m / 3 - 1
+    const int e_i = 3 * m + (tx < 9 ? 2 : 0), cy = m % 3 - 1, dz = 1 - m / 3;
+    const unsigned e_off = (unsigned)e_i * plane + (unsigned)pmod(y - cy, G.ny) * (unsigned)G.nx +
+                           (unsigned)(tx < 9 ? pmod(x0 - EC, G.nx) : pmod(x0 + TX, G.nx));
+    e_src = pop_slab(fin, G, pmod(z0 + dz, G.nz)) + e_off;
+    e_dst = (unsigned)__cvta_generic_to_shared(&S.fpop[m * T::TRIPLE + 3 * NT + (tx < 9 ? T::TAILE : 0) + EC * ty]);
+    e_zwrap = G.nz - 1 - dz;  // the call with this z (or z - nz) fetches the last plane: the next one is plane 0
   }
   auto prefetch_pull = [&](int z) {
     if (fast) {  // the boxes are on their way (after the block-wide hand-over)
       if (tx < 18) {
-        const int m = tx < 9 ? tx : tx - 9;  // population 3 m + 2 (c_ix = +1) or 3 m (c_ix = -1), c_iz = m / 3 - 1
-        const ST* sl = pop_slab(fin, G, m < 3 ? wrap_inc(z, G.nz) : m >= 6 ? wrap_dec(z, G.nz) : z);
-        cp_async_16(&S.fpop[m * T::TRIPLE + 3 * NT + (tx < 9 ? T::TAILE : 0) + EC * ty], sl + e_off);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(e_dst), "l"(e_src) : "memory");
+        const size_t slab = (size_t)Q * plane;
+        e_src += slab;
+        if (z == e_zwrap || z + G.nz == e_zwrap) e_src -= slab * (size_t)G.nz;
       }
       cp_async_commit();
       return;
