@@ -274,7 +274,7 @@ def measure_cuda(cfg, steps, warmup, *, local_rank=0, world=1, fp32=False, e2e=T
 # captures whose summaries are committed under profiles/ (bench.py does not read that folder).  A capture describes the
 # kernel as it was at the commit named; when a kernel changes, its entry is re-measured or removed (then `traffic` is null).
 NCU_TRAFFIC = {
-    ("k_lb_tp", "two", "fp64", 512): (62_372_635_000, "ncu --set full capture of k_lb_tp at commit ddf9676, profiles/r02_ncu_full.txt"),
+    ("k_lb_tp", "two", "fp64", 512): (62_318_549_000, "ncu --set full capture of k_lb_tp at commit 25120c8, profiles/r02_ncu_full.txt"),
     ("k_mr_step", "single", "fp64", 512): (22_290_332_000, "ncu --set full capture of k_mr_step at commit f434175, profiles/r02_ncu_full.txt (last block)"),
     ("k_lb", "single", "fp64", 512): (57_937_901_000, "ncu --set full capture of k_lb at commit f434175, profiles/r02_ncu_full.txt"),
 }
